@@ -1,0 +1,188 @@
+/*
+ * mlp_pipe.h -- C ABI of the CTA-pipelined chained GEMM for one B200 (sm_100a).
+ *
+ * What the library computes (the hot path of arxiv/paper_2607_07862, "CTA-Pipelining"):
+ *
+ *     A^0 = X;   A^l = bf16( act_l( A^{l-1} . W_l ) ),  l = 1..L;   Y = A^L
+ *
+ *   - "two-layer GEMM workload ... where the output of the first GEMM is directly
+ *     consumed by the subsequent GEMM"                 PAPER.md:107 (section III-B)
+ *   - "Y = XAB"; bf16 in / bf16 out, fp32 tensor-core accumulator
+ *                                                      PAPER.md:161
+ *   - every intermediate A^l is a kernel OUTPUT materialised in global memory
+ *     (arrow (1)), hence rounded to bf16 before the next layer reads it
+ *   - act_l is applied on the fp32 accumulator for l < L and is the identity for l = L
+ *     (the activation comes from BASELINE.json's configs; the paper omits it)
+ *
+ * and how: producer tiles (layer l) and consumer tiles (layer l+1) run at the same time
+ * inside ONE persistent launch.  A producer's epilogue stores its output tile and then
+ * publishes a ready counter (the paper's fence + scoreboard update, PAPER.md:95 steps
+ * (1)-(4)); a consumer's prologue polls the counters it depends on before it loads the
+ * intermediate (PAPER.md:95 step (5)); work is handed out by a global atomic ticket that
+ * orders all tiles of layer l before those of layer l+1 (the ordering knob of
+ * PAPER.md:99-101).  The same kernel also runs as the two baselines the paper compares
+ * against: stream-ordered SEQUENTIAL launches and static MICROBATCH
+ * chunk pipelining.
+ *
+ * Conventions for every entry point
+ *   - plain C, no exceptions cross the boundary; every function returns an MLP_* status
+ *     (0 = ok) unless stated otherwise.
+ *   - "device pointer" = address in the current CUDA device's global memory (e.g.
+ *     torch.Tensor.data_ptr()); "host pointer" = ordinary (ideally pinned) host memory.
+ *   - bf16 = the upper 16 bits of an IEEE binary32, stored as uint16_t.
+ *   - layouts: X [M x K] row-major (K contiguous); W_l [N_l x K_l] row-major (K_l
+ *     contiguous, i.e. nn.Linear.weight; logical W_l[k][n] = stored[n][k]); Y [M x N_L]
+ *     row-major.  The paper is silent on layout (its CUTLASS profiler chose).
+ *   - every K_l, N_l must be a multiple of 8 and every pointer 16-byte aligned (TMA
+ *     requirement); M >= 1 is arbitrary.
+ *   - the caller owns X, W_l, Y and the stream; the library owns the hidden activations
+ *     H_l, tickets, counters, the split-K workspace, tensor maps and internal streams.
+ *   - a handle is NOT re-entrant: runs on one handle must be stream-ordered after one
+ *     another (all counters are per handle).
+ *   - there is no CPU fallback: without an sm_100 device mlp_pipe_create fails with
+ *     MLP_ERR_UNSUPPORTED.
+ */
+#ifndef MLP_PIPE_H_
+#define MLP_PIPE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mlp_pipe mlp_pipe; /* opaque, library-owned */
+
+enum { MLP_OK = 0, MLP_ERR_INVALID = 1, MLP_ERR_UNSUPPORTED = 2, MLP_ERR_CUDA = 3, MLP_ERR_OOM = 4, MLP_ERR_TIMEOUT = 5 };
+
+/* dtype: bf16 in / bf16 out, fp32 accumulate -- the only one. */
+enum { MLP_BF16 = 0 };
+
+/* activation between layers (BASELINE.json configs; readings c1, c2).
+ * GELU_TANH: g(x) = 0.5 x (1 + tanh(sqrt(2/pi) (x + 0.044715 x^3))). */
+enum { MLP_ACT_NONE = 0, MLP_ACT_RELU = 1, MLP_ACT_GELU_TANH = 2 };
+
+/* execution mode */
+enum {
+    MLP_SEQUENTIAL = 0,   /* one launch per layer, stream-ordered, no flags      */
+    MLP_MICROBATCH = 1,   /* X split by rows into `chunks`; layer l of chunk i on stream l, after an
+                             event on layer l-1 of chunk i */
+    MLP_CTA_PIPELINED = 2 /* ONE persistent launch; tickets + ready counters */
+};
+
+#define MLP_MAX_LAYERS 8
+
+/* mlp_mode.flags */
+#define MLP_FLAG_TILE_MAJOR   0x1u  /* consumer layers hand out units tile-major (all K-slices of an
+                                       output tile adjacent) instead of K-slice-major (default)      */
+#define MLP_FLAG_DEBUG_DELAY  0x2u  /* test hook: producers of layer 1 sleep a pseudo-random time
+                                       before publishing (adversarial schedule for the protocol)     */
+#define MLP_FLAG_DEBUG_REVERSE 0x4u /* test hook: layer-1 units are handed out in reverse order       */
+#define MLP_FLAG_NO_W_EVICT_FIRST 0x8u /* do not tag weight loads L2 evict-first                      */
+
+typedef struct {
+    int kind;        /* MLP_SEQUENTIAL | MLP_MICROBATCH | MLP_CTA_PIPELINED                           */
+    int chunks;      /* MICROBATCH: number of row chunks, must divide M; ignored otherwise            */
+    float sm_split;  /* CTA_PIPELINED: fraction in (0,1] of the CTAs that draw layer-1 units first;
+                        the others start on layer 2 at once (prefetch W_2, poll for H).  1 = the pure
+                        single-ticket scheme.  0 is read as 1.                                         */
+    int tile_m;      /* tokens per tile (the tcgen05 N extent): 0 = auto, else a multiple of 16 <= 256 */
+    int tile_n;      /* weight rows per tile (the tcgen05 M extent): 0 or 128                          */
+    int tile_k;      /* contraction elements per pipeline stage: 0 or 64                               */
+    int stages;      /* shared-memory ring depth: 0 = as many as fit                                   */
+    int kslice_tiles;/* producer tiles per ready counter: 0 or 1 (one counter per (M-block, K-slice))  */
+    int split_k;     /* split of the contraction per output tile: 0 = auto, else applied to all layers */
+    unsigned flags;  /* MLP_FLAG_*                                                                     */
+    int split_k_layer[MLP_MAX_LAYERS]; /* per-layer override of split_k (0 = use split_k / auto)       */
+    int grid;        /* CTAs of the persistent launch: 0 = one per SM                                  */
+    int timeout_ms;  /* flag-poll watchdog: 0 = 2000 ms.  On expiry the kernel stops waiting, finishes
+                        with undefined output and the handle reports MLP_ERR_TIMEOUT                   */
+} mlp_mode;
+
+/*
+ * Create a handle for Y = act(X.W1).W2, X [M x K], W1 [N1 x K], W2 [N2 x N1].
+ * mode == NULL selects CTA_PIPELINED with every field auto.  Allocates all library-owned
+ * device memory here; *out is set only on MLP_OK.
+ * Errors: INVALID (null out, non-positive dims, dims not multiples of 8, bad mode fields,
+ * chunks not dividing M), UNSUPPORTED (no sm_100 device, dtype != MLP_BF16, tile shape outside
+ * the compiled set), OOM, CUDA.
+ */
+int mlp_pipe_create(mlp_pipe** out, int M, int K, int N1, int N2, int dtype, int act, const mlp_mode* mode);
+
+/*
+ * Same for an L-layer chain ("intermediate kernels act as both producers and
+ * consumers"; BASELINE.json configs[4]).  widths[0..n_layers] = K, N_1, ..., N_L (host
+ * pointer, copied).  1 <= n_layers <= MLP_MAX_LAYERS.  act after layers 1..L-1, none after L.
+ */
+int mlp_pipe_create_chain(mlp_pipe** out, int M, int n_layers, const int* widths, int dtype, int act,
+                          const mlp_mode* mode);
+
+/*
+ * One pass of the whole path.  X, W1, W2, Y: device pointers (layouts above).  cuda_stream:
+ * a cudaStream_t (NULL = the legacy default stream).  Asynchronous: enqueues on the stream
+ * and returns; no host synchronisation, no allocation.  Y is fully overwritten.
+ * Errors: INVALID (null / misaligned pointer), CUDA (launch failure, see last_error),
+ * TIMEOUT (a previous run on this handle hit the watchdog; the handle has been reset).
+ */
+int mlp_pipe_run(mlp_pipe* h, const void* X, const void* W1, const void* W2, void* Y, void* cuda_stream);
+
+/* Chain form: W = host array of n_layers device pointers. */
+int mlp_pipe_run_chain(mlp_pipe* h, const void* X, const void* const* W, void* Y, void* cuda_stream);
+
+/*
+ * End-to-end form with HOST buffers (bench.py's e2e leg): copies X and every W_l host->device
+ * into library-owned staging buffers, runs, copies Y device->host and synchronises the stream
+ * before returning.  X, W[l], Y are host pointers (pinned memory makes the copies asynchronous
+ * and fast; pageable memory works).  h2d_bytes / d2h_bytes (optional) receive the bytes moved.
+ */
+int mlp_pipe_run_host(mlp_pipe* h, const void* X, const void* const* W, void* Y, void* cuda_stream,
+                      size_t* h2d_bytes, size_t* d2h_bytes);
+
+/*
+ * Test hook: device pointer and size of hidden activation H_layer = A^layer, 1 <= layer < L
+ * ([M x N_layer] bf16 row-major).  Valid until destroy.
+ */
+int mlp_pipe_hidden(mlp_pipe* h, int layer, void** dev_ptr, size_t* bytes);
+
+/* Test hook: fill every H_l with the 16-bit pattern `pattern` (e.g. a bf16 NaN) on the stream,
+ * so that a consumer that reads H before it is published poisons Y. */
+int mlp_pipe_poison_hidden(mlp_pipe* h, uint16_t pattern, void* cuda_stream);
+
+/*
+ * Statistics of the most recent run.  Synchronises the device.  Fills as much of `out` as
+ * `bytes` allows.  Also the place where a watchdog expiry is reported (returns MLP_ERR_TIMEOUT).
+ */
+typedef struct {
+    int n_layers, grid, stages, tile_m;           /* resolved launch configuration                    */
+    int split_k[MLP_MAX_LAYERS];                  /* resolved per-layer split                         */
+    int units[MLP_MAX_LAYERS];                    /* work units per layer (tiles x split)             */
+    int producer_ctas;                            /* CTAs that start on layer 1 (sm_split)            */
+    uint32_t status;                              /* 0 ok, else device-side abort code                */
+    uint64_t runs;                                /* completed launches counted by the device epoch   */
+    uint64_t flag_stall_cycles_sum;               /* sum over CTAs of SM cycles spent polling flags    */
+    uint64_t flag_stall_cycles_max;               /* max over CTAs                                    */
+    uint64_t flag_polls;                          /* ld.acquire polls that found the slice not ready  */
+    uint64_t kernel_cycles_max;                   /* max over CTAs of the CTA's lifetime in SM cycles */
+    uint32_t units_done[MLP_MAX_LAYERS];          /* units executed per layer, summed over CTAs       */
+    uint32_t units_by_consumer_ctas[MLP_MAX_LAYERS]; /* of which by CTAs in the consumer-first group  */
+    uint32_t ready_ok;                            /* 1 if every ready counter / ticket / arrival
+                                                     counter holds its expected post-run value       */
+} mlp_stats;
+int mlp_pipe_stats(mlp_pipe* h, mlp_stats* out, size_t bytes);
+
+/* Free everything the handle owns (synchronises the device).  NULL is ignored. */
+void mlp_pipe_destroy(mlp_pipe* h);
+
+/* Static strings; never NULL. */
+const char* mlp_status_string(int status);
+/* Message of the last failing call on this handle (or on create, with h == NULL). */
+const char* mlp_pipe_last_error(const mlp_pipe* h);
+
+/* Library self-description: "mlp_pipe <version> sm_100a ..." */
+const char* mlp_pipe_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MLP_PIPE_H_ */

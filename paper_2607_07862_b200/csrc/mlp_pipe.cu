@@ -1,0 +1,593 @@
+// mlp_pipe.cu -- host side of the C ABI declared in include/mlp_pipe.h: handle, tensor maps,
+// resolution of the launch configuration, and the three modes' launch sequences.
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <cudaTypedefs.h>
+
+#include <algorithm>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/mlp_pipe.h"
+#include "kernel.cuh"
+
+using namespace mlp;
+
+static_assert(MLP_MAX_LAYERS == kMaxLayers, "header / kernel layer limit mismatch");
+static_assert(sizeof(KernelParams) <= 4000, "kernel parameter block too large");
+
+namespace {
+
+thread_local std::string g_create_error;
+
+struct TmapCacheEntry {
+    const void* ptr = nullptr;
+    CUtensorMap map;
+};
+
+constexpr int kTmapCache = 8;
+
+}  // namespace
+
+struct mlp_pipe {
+    int M = 0, L = 0;
+    int widths[kMaxLayers + 1] = {0};
+    int act = 0;
+    mlp_mode mode{};
+    int dev = 0, num_sms = 0;
+    // resolved configuration
+    int rows_per_launch = 0;  // M, or M / chunks
+    int tile_m = 0, m_blks = 0, stages = 0, grid = 0, producer_ctas = 0;
+    size_t smem_bytes = 0;
+    int split[kMaxLayers] = {0};
+    int tiles[kMaxLayers] = {0};
+    // device memory owned by the handle
+    __nv_bfloat16* H[kMaxLayers] = {nullptr};  // H[l] = output of layer l, l < L-1
+    float* ws[kMaxLayers] = {nullptr};
+    uint32_t* counters = nullptr;  // tickets | arrive | ready, all layers
+    size_t counters_words = 0;
+    uint32_t* ticket[kMaxLayers] = {nullptr};
+    uint32_t* arrive[kMaxLayers] = {nullptr};
+    uint32_t* ready[kMaxLayers] = {nullptr};
+    unsigned long long* epoch = nullptr;  // [kMaxLayers]
+    uint32_t* status = nullptr;
+    CtaStats* stats = nullptr;  // [kMaxLayers][grid]
+    // staging for run_host
+    void* stage_X = nullptr;
+    void* stage_W[kMaxLayers] = {nullptr};
+    void* stage_Y = nullptr;
+    // launch template + tensor-map caches
+    KernelParams base{};
+    TmapCacheEntry cache_w[kMaxLayers][kTmapCache];
+    TmapCacheEntry cache_x[kTmapCache];
+    int cache_w_next[kMaxLayers] = {0};
+    int cache_x_next = 0;
+    // MICROBATCH plumbing
+    std::vector<cudaStream_t> side;
+    cudaEvent_t ev_fork = nullptr;
+    std::vector<cudaEvent_t> ev_done;  // [L][chunks]
+    bool poisoned_state = false;       // a watchdog expiry was seen: counters must be reset
+    unsigned long long runs = 0;
+    std::string last_error;
+};
+
+namespace {
+
+PFN_cuTensorMapEncodeTiled_v12000 get_encode() {
+    static PFN_cuTensorMapEncodeTiled_v12000 fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(p);
+    }
+    return fn;
+}
+
+int fail(mlp_pipe* h, int code, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (h) h->last_error = buf;
+    else g_create_error = buf;
+    return code;
+}
+
+#define CUDA_TRY(h, expr)                                                                         \
+    do {                                                                                          \
+        cudaError_t e_ = (expr);                                                                  \
+        if (e_ != cudaSuccess)                                                                    \
+            return fail(h, e_ == cudaErrorMemoryAllocation ? MLP_ERR_OOM : MLP_ERR_CUDA, "%s: %s", #expr, \
+                        cudaGetErrorString(e_));                                                  \
+    } while (0)
+
+// bf16 row-major [rows x cols] (cols contiguous), box = [box_rows x 64], 128-byte swizzle.
+int encode_2d(mlp_pipe* h, CUtensorMap* out, const void* ptr, int rows, int cols, int box_rows) {
+    auto enc = get_encode();
+    if (!enc) return fail(h, MLP_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
+    cuuint64_t gdim[2] = {static_cast<cuuint64_t>(cols), static_cast<cuuint64_t>(rows)};
+    cuuint64_t gstr[1] = {static_cast<cuuint64_t>(cols) * 2};
+    cuuint32_t box[2] = {static_cast<cuuint32_t>(kTileK), static_cast<cuuint32_t>(box_rows)};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = enc(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr), gdim, gstr, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(h, MLP_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d) rows=%d cols=%d box_rows=%d ptr=%p",
+                                       static_cast<int>(r), rows, cols, box_rows, ptr);
+    return MLP_OK;
+}
+
+int round_up(int a, int b) { return (a + b - 1) / b * b; }
+int ceil_div(int a, int b) { return (a + b - 1) / b; }
+
+int validate_mode(const mlp_mode& m, int M) {
+    if (m.kind < MLP_SEQUENTIAL || m.kind > MLP_CTA_PIPELINED) return MLP_ERR_INVALID;
+    if (m.kind == MLP_MICROBATCH && (m.chunks < 1 || M % m.chunks != 0)) return MLP_ERR_INVALID;
+    if (m.sm_split < 0.0f || m.sm_split > 1.0f) return MLP_ERR_INVALID;
+    if (m.tile_m < 0 || m.tile_m % 16 != 0) return MLP_ERR_INVALID;
+    if (m.stages < 0 || m.split_k < 0 || m.grid < 0 || m.timeout_ms < 0) return MLP_ERR_INVALID;
+    for (int l = 0; l < kMaxLayers; ++l)
+        if (m.split_k_layer[l] < 0) return MLP_ERR_INVALID;
+    if (m.tile_m > 256 || (m.tile_n != 0 && m.tile_n != kTileN) || (m.tile_k != 0 && m.tile_k != kTileK) ||
+        (m.kslice_tiles != 0 && m.kslice_tiles != 1))
+        return MLP_ERR_UNSUPPORTED;
+    return MLP_OK;
+}
+
+// The launch configuration.
+void resolve(mlp_pipe* h) {
+    const mlp_mode& m = h->mode;
+    h->rows_per_launch = m.kind == MLP_MICROBATCH ? h->M / m.chunks : h->M;
+    if (m.tile_m > 0) {
+        h->tile_m = m.tile_m;
+        h->m_blks = ceil_div(h->rows_per_launch, h->tile_m);
+    } else {
+        h->m_blks = ceil_div(h->rows_per_launch, 256);
+        h->tile_m = round_up(ceil_div(h->rows_per_launch, h->m_blks), 16);
+    }
+    const int stage_bytes = kWTileBytes + h->tile_m * kTileK * 2;
+    const int max_smem = 227 * 1024;
+    int st = (max_smem - kCtrlBytes - 1024) / stage_bytes;
+    st = std::min(st, kMaxStages);
+    if (m.stages > 0) st = std::min(st, m.stages);
+    h->stages = std::max(st, 2);
+    h->smem_bytes = static_cast<size_t>(h->stages) * stage_bytes + kCtrlBytes + 1024;
+    h->grid = m.grid > 0 ? std::min(m.grid, h->num_sms) : h->num_sms;
+    const float s = (m.sm_split <= 0.0f) ? 1.0f : m.sm_split;
+    h->producer_ctas = h->grid;
+    if (m.kind == MLP_CTA_PIPELINED && h->L > 1 && s < 1.0f)
+        h->producer_ctas = std::min(h->grid, std::max(1, static_cast<int>(h->grid * s + 0.5f)));
+    // split-K: enough units to keep every SM streaming weights, but never so fine that the fp32
+    // partials rival the weight bytes of a unit
+    const int kb_min = h->tile_m <= 32 ? 8 : h->tile_m <= 64 ? 16 : h->tile_m <= 128 ? 32 : 64;
+    const int target_units = 3 * h->grid;
+    for (int l = 0; l < h->L; ++l) {
+        const int kb_total = ceil_div(h->widths[l], kTileK);
+        const int n_blks = ceil_div(h->widths[l + 1], kTileN);
+        h->tiles[l] = n_blks * h->m_blks;
+        int sp = m.split_k_layer[l] > 0 ? m.split_k_layer[l] : m.split_k;
+        if (sp <= 0) {
+            sp = ceil_div(target_units, h->tiles[l]);
+            sp = std::min(sp, std::max(1, kb_total / kb_min));
+        }
+        h->split[l] = std::max(1, std::min(sp, kb_total));
+    }
+}
+
+int build_base_params(mlp_pipe* h) {
+    KernelParams& P = h->base;
+    memset(&P, 0, sizeof P);
+    for (int l = 0; l < h->L; ++l) {
+        LayerParams& Lp = P.layer[l];
+        Lp.K = h->widths[l];
+        Lp.N = h->widths[l + 1];
+        Lp.kb_total = ceil_div(Lp.K, kTileK);
+        Lp.n_blks = ceil_div(Lp.N, kTileN);
+        Lp.split = h->split[l];
+        Lp.units = h->tiles[l] * h->split[l];
+        Lp.drawers = h->grid;
+        Lp.act = l < h->L - 1 ? h->act : kActNone;
+        Lp.publish = l < h->L - 1 ? 1 : 0;
+        Lp.out = l < h->L - 1 ? h->H[l] : nullptr;  // last layer: caller's Y, patched per run
+        Lp.ws = h->ws[l];
+        Lp.ticket = h->ticket[l];
+        Lp.arrive = h->arrive[l];
+        Lp.ready = h->ready[l];
+        if (l > 0) {
+            int rc = encode_2d(h, &P.tm_a[l], h->H[l - 1], h->M, h->widths[l], h->tile_m);
+            if (rc) return rc;
+        }
+    }
+    P.tile_m = h->tile_m;
+    P.m_blks = h->m_blks;
+    P.stages = h->stages;
+    P.flags = h->mode.flags;
+    P.status = h->status;
+    P.timeout_ns = static_cast<unsigned long long>(h->mode.timeout_ms > 0 ? h->mode.timeout_ms : 2000) * 1000000ull;
+    return MLP_OK;
+}
+
+int reset_state(mlp_pipe* h, cudaStream_t s) {
+    CUDA_TRY(h, cudaMemsetAsync(h->counters, 0, h->counters_words * sizeof(uint32_t), s));
+    CUDA_TRY(h, cudaMemsetAsync(h->epoch, 0, kMaxLayers * sizeof(unsigned long long), s));
+    CUDA_TRY(h, cudaMemsetAsync(h->status, 0, sizeof(uint32_t), s));
+    CUDA_TRY(h, cudaMemsetAsync(h->stats, 0, sizeof(CtaStats) * kMaxLayers * h->grid, s));
+    return MLP_OK;
+}
+
+int lookup_tmap(mlp_pipe* h, TmapCacheEntry* cache, int* next, const void* ptr, int rows, int cols, int box_rows,
+                CUtensorMap* out) {
+    for (int i = 0; i < kTmapCache; ++i)
+        if (cache[i].ptr == ptr) {
+            *out = cache[i].map;
+            return MLP_OK;
+        }
+    TmapCacheEntry& e = cache[*next];
+    int rc = encode_2d(h, &e.map, ptr, rows, cols, box_rows);
+    if (rc) {
+        e.ptr = nullptr;
+        return rc;
+    }
+    e.ptr = ptr;
+    *out = e.map;
+    *next = (*next + 1) % kTmapCache;
+    return MLP_OK;
+}
+
+int launch(mlp_pipe* h, const KernelParams& P, cudaStream_t s) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(h->grid);
+    cfg.blockDim = dim3(kThreads);
+    cfg.dynamicSmemBytes = h->smem_bytes;
+    cfg.stream = s;
+    cfg.attrs = nullptr;
+    cfg.numAttrs = 0;
+    CUDA_TRY(h, cudaLaunchKernelEx(&cfg, mlp_pipe_kernel, P));
+    return MLP_OK;
+}
+
+int create_impl(mlp_pipe** out, int M, int L, const int* widths, int dtype, int act, const mlp_mode* mode) {
+    if (!out) return fail(nullptr, MLP_ERR_INVALID, "out is NULL");
+    *out = nullptr;
+    if (!widths || L < 1 || L > kMaxLayers || M < 1) return fail(nullptr, MLP_ERR_INVALID, "bad M / n_layers / widths");
+    if (dtype != MLP_BF16) return fail(nullptr, MLP_ERR_UNSUPPORTED, "dtype %d not supported (bf16 only)", dtype);
+    if (act < MLP_ACT_NONE || act > MLP_ACT_GELU_TANH) return fail(nullptr, MLP_ERR_INVALID, "bad act %d", act);
+    for (int l = 0; l <= L; ++l)
+        if (widths[l] < 8 || widths[l] % 8 != 0)
+            return fail(nullptr, MLP_ERR_INVALID, "width[%d] = %d must be a positive multiple of 8", l, widths[l]);
+    mlp_mode m{};
+    if (mode) m = *mode;
+    else m.kind = MLP_CTA_PIPELINED;
+    int rc = validate_mode(m, M);
+    if (rc) return fail(nullptr, rc, "invalid or unsupported mlp_mode");
+
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return fail(nullptr, MLP_ERR_UNSUPPORTED, "no CUDA device");
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return fail(nullptr, MLP_ERR_UNSUPPORTED, "no CUDA device");
+    if (prop.major != 10) return fail(nullptr, MLP_ERR_UNSUPPORTED, "device is sm_%d%d, this library is sm_100a only", prop.major, prop.minor);
+
+    mlp_pipe* h = new (std::nothrow) mlp_pipe();
+    if (!h) return fail(nullptr, MLP_ERR_OOM, "host allocation failed");
+    h->M = M;
+    h->L = L;
+    for (int l = 0; l <= L; ++l) h->widths[l] = widths[l];
+    h->act = act;
+    h->mode = m;
+    h->dev = dev;
+    h->num_sms = prop.multiProcessorCount;
+    resolve(h);
+
+#define CREATE_TRY(expr)                                                             \
+    do {                                                                             \
+        cudaError_t e_ = (expr);                                                     \
+        if (e_ != cudaSuccess) {                                                     \
+            int code_ = e_ == cudaErrorMemoryAllocation ? MLP_ERR_OOM : MLP_ERR_CUDA; \
+            fail(nullptr, code_, "%s: %s", #expr, cudaGetErrorString(e_));           \
+            cudaGetLastError();                                                      \
+            mlp_pipe_destroy(h);                                                     \
+            return code_;                                                            \
+        }                                                                            \
+    } while (0)
+
+    CREATE_TRY(cudaFuncSetAttribute(mlp_pipe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(h->smem_bytes)));
+    for (int l = 0; l < L - 1; ++l) CREATE_TRY(cudaMalloc(&h->H[l], static_cast<size_t>(M) * widths[l + 1] * 2));
+    size_t words = 0;
+    for (int l = 0; l < L; ++l) words += 32 + 2 * static_cast<size_t>(round_up(h->tiles[l], 32));
+    h->counters_words = words;
+    CREATE_TRY(cudaMalloc(&h->counters, words * sizeof(uint32_t)));
+    {
+        uint32_t* p = h->counters;
+        for (int l = 0; l < L; ++l) {
+            h->ticket[l] = p;  // own 128-byte line
+            p += 32;
+            h->arrive[l] = p;
+            p += round_up(h->tiles[l], 32);
+            h->ready[l] = p;
+            p += round_up(h->tiles[l], 32);
+        }
+    }
+    for (int l = 0; l < L; ++l)
+        if (h->split[l] > 1)
+            CREATE_TRY(cudaMalloc(&h->ws[l], static_cast<size_t>(h->tiles[l]) * h->split[l] * h->tile_m * kTileN * sizeof(float)));
+    CREATE_TRY(cudaMalloc(&h->epoch, kMaxLayers * sizeof(unsigned long long)));
+    CREATE_TRY(cudaMalloc(&h->status, sizeof(uint32_t)));
+    CREATE_TRY(cudaMalloc(&h->stats, sizeof(CtaStats) * kMaxLayers * h->grid));
+    if (m.kind == MLP_MICROBATCH) {
+        h->side.resize(L, nullptr);
+        for (int l = 0; l < L; ++l) CREATE_TRY(cudaStreamCreateWithFlags(&h->side[l], cudaStreamNonBlocking));
+        CREATE_TRY(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
+        h->ev_done.resize(static_cast<size_t>(L) * m.chunks, nullptr);
+        for (auto& e : h->ev_done) CREATE_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    }
+    rc = reset_state(h, nullptr);
+    if (rc == MLP_OK) rc = build_base_params(h);
+    if (rc == MLP_OK && cudaDeviceSynchronize() != cudaSuccess) rc = MLP_ERR_CUDA;
+    if (rc) {
+        g_create_error = h->last_error;
+        mlp_pipe_destroy(h);
+        return rc;
+    }
+    *out = h;
+    return MLP_OK;
+#undef CREATE_TRY
+}
+
+int check_ptr(mlp_pipe* h, const void* p, const char* name) {
+    if (!p) return fail(h, MLP_ERR_INVALID, "%s is NULL", name);
+    if (reinterpret_cast<uintptr_t>(p) & 15u) return fail(h, MLP_ERR_INVALID, "%s is not 16-byte aligned", name);
+    return MLP_OK;
+}
+
+int run_impl(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStream_t s) {
+    int rc;
+    if ((rc = check_ptr(h, X, "X"))) return rc;
+    if ((rc = check_ptr(h, Y, "Y"))) return rc;
+    if (!W) return fail(h, MLP_ERR_INVALID, "W is NULL");
+    for (int l = 0; l < h->L; ++l)
+        if ((rc = check_ptr(h, W[l], "W[l]"))) return rc;
+    if (h->poisoned_state) {
+        CUDA_TRY(h, cudaDeviceSynchronize());
+        if ((rc = reset_state(h, s))) return rc;
+        h->poisoned_state = false;
+        return fail(h, MLP_ERR_TIMEOUT, "a previous run hit the flag watchdog; the handle has been reset");
+    }
+    KernelParams P = h->base;
+    if ((rc = lookup_tmap(h, h->cache_x, &h->cache_x_next, X, h->M, h->widths[0], h->tile_m, &P.tm_a[0]))) return rc;
+    for (int l = 0; l < h->L; ++l)
+        if ((rc = lookup_tmap(h, h->cache_w[l], &h->cache_w_next[l], W[l], h->widths[l + 1], h->widths[l], kTileN, &P.tm_w[l])))
+            return rc;
+    P.layer[h->L - 1].out = static_cast<__nv_bfloat16*>(Y);
+
+    const int kind = h->mode.kind;
+    if (kind == MLP_CTA_PIPELINED) {
+        // one persistent launch; tickets order all units of layer l before those of layer l+1
+        P.layer_begin = 0;
+        P.layer_end = h->L;
+        P.m_off = 0;
+        P.m_end = h->M;
+        P.wait_flags = 1;
+        P.producer_ctas = h->producer_ctas;
+        P.layer[0].drawers = h->producer_ctas;
+        P.epoch_counter = h->epoch;
+        P.stats = h->stats;
+        if ((rc = launch(h, P, s))) return rc;
+    } else if (kind == MLP_SEQUENTIAL) {
+        // consecutive kernels, stream order is the only dependency mechanism
+        for (int l = 0; l < h->L; ++l) {
+            P.layer_begin = l;
+            P.layer_end = l + 1;
+            P.m_off = 0;
+            P.m_end = h->M;
+            P.wait_flags = 0;
+            P.producer_ctas = h->grid;
+            P.epoch_counter = h->epoch + l;
+            P.stats = h->stats + static_cast<size_t>(l) * h->grid;
+            if ((rc = launch(h, P, s))) return rc;
+        }
+    } else {
+        // PAPER.md:169-173, Fig. 3a: X split by rows into chunks; layer l of chunk i runs on stream l after
+        // layer l-1 of chunk i, so layer l-1 of chunk i+1 overlaps it
+        const int chunks = h->mode.chunks;
+        const int rows = h->rows_per_launch;
+        CUDA_TRY(h, cudaEventRecord(h->ev_fork, s));
+        for (int l = 0; l < h->L; ++l) CUDA_TRY(h, cudaStreamWaitEvent(h->side[l], h->ev_fork, 0));
+        for (int c = 0; c < chunks; ++c)
+            for (int l = 0; l < h->L; ++l) {
+                if (l > 0) CUDA_TRY(h, cudaStreamWaitEvent(h->side[l], h->ev_done[static_cast<size_t>(l - 1) * chunks + c], 0));
+                P.layer_begin = l;
+                P.layer_end = l + 1;
+                P.m_off = c * rows;
+                P.m_end = (c + 1) * rows;
+                P.wait_flags = 0;
+                P.producer_ctas = h->grid;
+                P.epoch_counter = h->epoch + l;
+                P.stats = h->stats + static_cast<size_t>(l) * h->grid;
+                if ((rc = launch(h, P, h->side[l]))) return rc;
+                CUDA_TRY(h, cudaEventRecord(h->ev_done[static_cast<size_t>(l) * chunks + c], h->side[l]));
+            }
+        CUDA_TRY(h, cudaStreamWaitEvent(s, h->ev_done[static_cast<size_t>(h->L - 1) * chunks + chunks - 1], 0));
+    }
+    h->runs++;
+    return MLP_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int mlp_pipe_create(mlp_pipe** out, int M, int K, int N1, int N2, int dtype, int act, const mlp_mode* mode) {
+    const int widths[3] = {K, N1, N2};
+    return create_impl(out, M, 2, widths, dtype, act, mode);
+}
+
+int mlp_pipe_create_chain(mlp_pipe** out, int M, int n_layers, const int* widths, int dtype, int act,
+                          const mlp_mode* mode) {
+    return create_impl(out, M, n_layers, widths, dtype, act, mode);
+}
+
+int mlp_pipe_run(mlp_pipe* h, const void* X, const void* W1, const void* W2, void* Y, void* cuda_stream) {
+    if (!h) return MLP_ERR_INVALID;
+    if (h->L != 2) return fail(h, MLP_ERR_INVALID, "mlp_pipe_run needs a 2-layer handle (use mlp_pipe_run_chain)");
+    const void* W[2] = {W1, W2};
+    return run_impl(h, X, W, Y, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int mlp_pipe_run_chain(mlp_pipe* h, const void* X, const void* const* W, void* Y, void* cuda_stream) {
+    if (!h) return MLP_ERR_INVALID;
+    return run_impl(h, X, W, Y, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int mlp_pipe_run_host(mlp_pipe* h, const void* X, const void* const* W, void* Y, void* cuda_stream, size_t* h2d_bytes,
+                      size_t* d2h_bytes) {
+    if (!h) return MLP_ERR_INVALID;
+    if (!X || !W || !Y) return fail(h, MLP_ERR_INVALID, "NULL host pointer");
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    const size_t xb = static_cast<size_t>(h->M) * h->widths[0] * 2;
+    const size_t yb = static_cast<size_t>(h->M) * h->widths[h->L] * 2;
+    if (!h->stage_X) {
+        CUDA_TRY(h, cudaMalloc(&h->stage_X, xb));
+        CUDA_TRY(h, cudaMalloc(&h->stage_Y, yb));
+        for (int l = 0; l < h->L; ++l)
+            CUDA_TRY(h, cudaMalloc(&h->stage_W[l], static_cast<size_t>(h->widths[l]) * h->widths[l + 1] * 2));
+    }
+    size_t in = xb;
+    CUDA_TRY(h, cudaMemcpyAsync(h->stage_X, X, xb, cudaMemcpyHostToDevice, s));
+    for (int l = 0; l < h->L; ++l) {
+        if (!W[l]) return fail(h, MLP_ERR_INVALID, "W[%d] is NULL", l);
+        const size_t wb = static_cast<size_t>(h->widths[l]) * h->widths[l + 1] * 2;
+        CUDA_TRY(h, cudaMemcpyAsync(h->stage_W[l], W[l], wb, cudaMemcpyHostToDevice, s));
+        in += wb;
+    }
+    int rc = run_impl(h, h->stage_X, h->stage_W, h->stage_Y, s);
+    if (rc) return rc;
+    CUDA_TRY(h, cudaMemcpyAsync(Y, h->stage_Y, yb, cudaMemcpyDeviceToHost, s));
+    CUDA_TRY(h, cudaStreamSynchronize(s));
+    if (h2d_bytes) *h2d_bytes = in;
+    if (d2h_bytes) *d2h_bytes = yb;
+    return MLP_OK;
+}
+
+int mlp_pipe_hidden(mlp_pipe* h, int layer, void** dev_ptr, size_t* bytes) {
+    if (!h) return MLP_ERR_INVALID;
+    if (layer < 1 || layer >= h->L || !dev_ptr || !bytes) return fail(h, MLP_ERR_INVALID, "bad layer %d (1 <= layer < %d)", layer, h->L);
+    *dev_ptr = h->H[layer - 1];
+    *bytes = static_cast<size_t>(h->M) * h->widths[layer] * 2;
+    return MLP_OK;
+}
+
+int mlp_pipe_poison_hidden(mlp_pipe* h, uint16_t pattern, void* cuda_stream) {
+    if (!h) return MLP_ERR_INVALID;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    for (int l = 0; l < h->L - 1; ++l) {
+        const size_t n = static_cast<size_t>(h->M) * h->widths[l + 1];
+        CUDA_TRY(h, cudaMemset2DAsync(h->H[l], 2, pattern & 0xff, 1, n, s));
+        CUDA_TRY(h, cudaMemset2DAsync(reinterpret_cast<uint8_t*>(h->H[l]) + 1, 2, pattern >> 8, 1, n, s));
+    }
+    return MLP_OK;
+}
+
+int mlp_pipe_stats(mlp_pipe* h, mlp_stats* out, size_t bytes) {
+    if (!h || !out) return MLP_ERR_INVALID;
+    CUDA_TRY(h, cudaDeviceSynchronize());
+    mlp_stats st;
+    memset(&st, 0, sizeof st);
+    st.n_layers = h->L;
+    st.grid = h->grid;
+    st.stages = h->stages;
+    st.tile_m = h->tile_m;
+    st.producer_ctas = h->producer_ctas;
+    for (int l = 0; l < h->L; ++l) {
+        st.split_k[l] = h->split[l];
+        st.units[l] = h->tiles[l] * h->split[l];
+    }
+    CUDA_TRY(h, cudaMemcpy(&st.status, h->status, sizeof(uint32_t), cudaMemcpyDeviceToHost));
+    unsigned long long ep[kMaxLayers];
+    CUDA_TRY(h, cudaMemcpy(ep, h->epoch, sizeof ep, cudaMemcpyDeviceToHost));
+    st.runs = ep[0] / h->grid;
+    const int classes = h->mode.kind == MLP_CTA_PIPELINED ? 1 : h->L;
+    std::vector<CtaStats> cs(static_cast<size_t>(classes) * h->grid);
+    CUDA_TRY(h, cudaMemcpy(cs.data(), h->stats, cs.size() * sizeof(CtaStats), cudaMemcpyDeviceToHost));
+    for (int c = 0; c < classes; ++c)
+        for (int b = 0; b < h->grid; ++b) {
+            const CtaStats& s = cs[static_cast<size_t>(c) * h->grid + b];
+            st.flag_stall_cycles_sum += s.stall_cycles;
+            st.flag_stall_cycles_max = std::max<uint64_t>(st.flag_stall_cycles_max, s.stall_cycles);
+            st.flag_polls += s.polls;
+            st.kernel_cycles_max = std::max<uint64_t>(st.kernel_cycles_max, s.cycles);
+            for (int l = 0; l < h->L; ++l) {
+                st.units_done[l] += s.units[l];
+                if (b >= h->producer_ctas) st.units_by_consumer_ctas[l] += s.units[l];
+            }
+        }
+    // post-run invariants of the protocol state
+    std::vector<uint32_t> cw(h->counters_words);
+    CUDA_TRY(h, cudaMemcpy(cw.data(), h->counters, cw.size() * sizeof(uint32_t), cudaMemcpyDeviceToHost));
+    bool ok = st.status == 0;
+    for (int l = 0; l < h->L && ok; ++l) {
+        const unsigned long long e = (h->mode.kind == MLP_CTA_PIPELINED ? ep[0] : ep[l]) / h->grid;
+        const int drawers = (h->mode.kind == MLP_CTA_PIPELINED && l == 0) ? h->producer_ctas : h->grid;
+        const uint32_t* tk = cw.data() + (h->ticket[l] - h->counters);
+        const uint32_t* ar = cw.data() + (h->arrive[l] - h->counters);
+        const uint32_t* rd = cw.data() + (h->ready[l] - h->counters);
+        ok = ok && tk[0] == static_cast<uint32_t>(e * static_cast<unsigned long long>(st.units[l] + drawers));
+        for (int t = 0; t < h->tiles[l] && ok; ++t) {
+            ok = ok && ar[t] == (h->split[l] > 1 ? static_cast<uint32_t>(e * h->split[l]) : 0u);
+            ok = ok && rd[t] == (l < h->L - 1 ? static_cast<uint32_t>(e) : 0u);
+        }
+    }
+    st.ready_ok = ok ? 1u : 0u;
+    memcpy(out, &st, std::min(bytes, sizeof st));
+    if (st.status != 0) {
+        h->poisoned_state = true;
+        return fail(h, MLP_ERR_TIMEOUT, "flag-poll watchdog expired on the device (status %u)", st.status);
+    }
+    return MLP_OK;
+}
+
+void mlp_pipe_destroy(mlp_pipe* h) {
+    if (!h) return;
+    cudaDeviceSynchronize();
+    for (int l = 0; l < kMaxLayers; ++l) {
+        if (h->H[l]) cudaFree(h->H[l]);
+        if (h->ws[l]) cudaFree(h->ws[l]);
+        if (h->stage_W[l]) cudaFree(h->stage_W[l]);
+    }
+    if (h->counters) cudaFree(h->counters);
+    if (h->epoch) cudaFree(h->epoch);
+    if (h->status) cudaFree(h->status);
+    if (h->stats) cudaFree(h->stats);
+    if (h->stage_X) cudaFree(h->stage_X);
+    if (h->stage_Y) cudaFree(h->stage_Y);
+    for (auto s : h->side)
+        if (s) cudaStreamDestroy(s);
+    if (h->ev_fork) cudaEventDestroy(h->ev_fork);
+    for (auto e : h->ev_done)
+        if (e) cudaEventDestroy(e);
+    delete h;
+}
+
+const char* mlp_status_string(int status) {
+    switch (status) {
+        case MLP_OK: return "ok";
+        case MLP_ERR_INVALID: return "invalid argument";
+        case MLP_ERR_UNSUPPORTED: return "unsupported device, dtype or tile shape";
+        case MLP_ERR_CUDA: return "CUDA error";
+        case MLP_ERR_OOM: return "out of memory";
+        case MLP_ERR_TIMEOUT: return "flag-poll watchdog expired";
+        default: return "unknown status";
+    }
+}
+
+const char* mlp_pipe_last_error(const mlp_pipe* h) { return h ? h->last_error.c_str() : g_create_error.c_str(); }
+
+const char* mlp_pipe_version(void) { return "mlp_pipe 0.1 sm_100a tcgen05/TMA bf16 (CTA-pipelined chained GEMM)"; }
+
+}  // extern "C"
