@@ -171,6 +171,26 @@ typedef struct {
 } mlp_stats;
 int mlp_pipe_stats(mlp_pipe* h, mlp_stats* out, size_t bytes);
 
+/*
+ * Profiling hook (the paper's in-kernel timestamp instrumentation): per-CTA records
+ * of the most recent launch of launch class `cls` (0 for CTA_PIPELINED; the layer index for
+ * SEQUENTIAL / MICROBATCH).  Copies min(max_records, grid) records to the host array `out` and
+ * returns the number copied through *n_out.  Synchronises the device.
+ */
+typedef struct {
+    uint64_t flag_stall_cycles;   /* SM cycles the consumer prologue spent polling                        */
+    uint64_t flag_polls;          /* unsuccessful polls                                                   */
+    uint64_t cycles;              /* CTA lifetime in SM cycles                                            */
+    uint64_t ts[8];               /* globaltimer ns: 0 CTA start, 1 setup done, 2 first ticket decoded,
+                                     3 first weight TMA issued, 4 first stage landed, 5 first accumulator
+                                     complete, 6 first unit stored (+published), 7 CTA exit               */
+    uint64_t wait[6];             /* SM cycles blocked: 0 weight loader on a free stage, 1 unused, 2 MMA on
+                                     operands, 3 MMA on a free accumulator, 4 epilogue on an accumulator,
+                                     5 split-K reducer on the other slices' partials                      */
+    uint32_t units[MLP_MAX_LAYERS]; /* units this CTA executed, per layer                                 */
+} mlp_cta_record;
+int mlp_pipe_cta_records(mlp_pipe* h, int cls, mlp_cta_record* out, int max_records, int* n_out);
+
 /* Free everything the handle owns (synchronises the device).  NULL is ignored. */
 void mlp_pipe_destroy(mlp_pipe* h);
 

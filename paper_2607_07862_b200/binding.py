@@ -25,7 +25,7 @@ MLP_FLAG_TILE_MAJOR, MLP_FLAG_DEBUG_DELAY, MLP_FLAG_DEBUG_REVERSE, MLP_FLAG_NO_W
 EXPORTS = [
     "mlp_pipe_create", "mlp_pipe_create_chain", "mlp_pipe_run", "mlp_pipe_run_chain", "mlp_pipe_run_host",
     "mlp_pipe_hidden", "mlp_pipe_poison_hidden", "mlp_pipe_stats", "mlp_pipe_destroy", "mlp_status_string",
-    "mlp_pipe_last_error", "mlp_pipe_version",
+    "mlp_pipe_last_error", "mlp_pipe_version", "mlp_pipe_cta_records",
 ]
 
 
@@ -48,6 +48,13 @@ class mlp_stats(ctypes.Structure):
         ("flag_polls", ctypes.c_uint64), ("kernel_cycles_max", ctypes.c_uint64),
         ("units_done", ctypes.c_uint32 * MLP_MAX_LAYERS),
         ("units_by_consumer_ctas", ctypes.c_uint32 * MLP_MAX_LAYERS), ("ready_ok", ctypes.c_uint32),
+    ]
+
+
+class mlp_cta_record(ctypes.Structure):
+    _fields_ = [
+        ("flag_stall_cycles", ctypes.c_uint64), ("flag_polls", ctypes.c_uint64), ("cycles", ctypes.c_uint64),
+        ("ts", ctypes.c_uint64 * 8), ("wait", ctypes.c_uint64 * 6), ("units", ctypes.c_uint32 * MLP_MAX_LAYERS),
     ]
 
 
@@ -87,6 +94,8 @@ def load(build_if_missing: bool = True):
     lib.mlp_pipe_poison_hidden.argtypes = [vp, ctypes.c_uint16, vp]
     lib.mlp_pipe_stats.restype = ci
     lib.mlp_pipe_stats.argtypes = [vp, ctypes.POINTER(mlp_stats), ctypes.c_size_t]
+    lib.mlp_pipe_cta_records.restype = ci
+    lib.mlp_pipe_cta_records.argtypes = [vp, ci, ctypes.POINTER(mlp_cta_record), ci, ctypes.POINTER(ci)]
     lib.mlp_pipe_destroy.restype = None
     lib.mlp_pipe_destroy.argtypes = [vp]
     lib.mlp_status_string.restype = ctypes.c_char_p
@@ -204,6 +213,12 @@ class MlpPipe:
         s = mlp_stats()
         _check(self._lib.mlp_pipe_stats(self._h, ctypes.byref(s), ctypes.sizeof(s)), self._h)
         return s
+
+    def cta_records(self, cls: int = 0, max_records: int = 256):
+        arr = (mlp_cta_record * max_records)()
+        n = ctypes.c_int()
+        _check(self._lib.mlp_pipe_cta_records(self._h, cls, arr, max_records, ctypes.byref(n)), self._h)
+        return [arr[i] for i in range(n.value)]
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h.value:

@@ -50,10 +50,10 @@ struct LayerParams {
     int n_blks;    // ceil(N / 128)
     int split;     // split of the contraction per output tile
     int units;     // n_blks * m_blks * split
-    int drawers;   // CTAs that draw tickets of this layer in one launch
+    int ticket_inc;  // what one launch adds to the ticket counter: units + CTAs arriving from the layer before
+    int ticket_off;  // unit index of the first atomically drawn ticket (= units handed out statically)
     int act;       // activation on this layer's output
     int publish;   // 1 if a later layer consumes this layer's output
-    int pad_;
     __nv_bfloat16* out;  // [M x N] row-major
     float* ws;           // split-K partials [tile][split][tile_m][128]
     uint32_t* ticket;    // 1 monotone counter
@@ -65,6 +65,11 @@ struct CtaStats {
     unsigned long long stall_cycles;
     unsigned long long polls;
     unsigned long long cycles;
+    unsigned long long ts[8];  // globaltimer ns: 0 start, 1 setup done, 2 first ticket, 3 first W TMA issued,
+                               // 4 first stage landed, 5 first accumulator ready, 6 first unit stored, 7 exit
+    unsigned long long wait[6];  // SM cycles blocked: 0 W loader on a free stage, 1 (unused, see stall_cycles),
+                                 // 2 MMA on operands, 3 MMA on a free accumulator, 4 epilogue on an accumulator,
+                                 // 5 split-K reducer on the other slices' partials
     uint32_t units[kMaxLayers];
 };
 
@@ -106,6 +111,35 @@ __device__ __forceinline__ float ld_cg_f32(const float* p) {
     return v;
 }
 
+__device__ __forceinline__ void mbar_wait_timed(uint32_t bar, uint32_t parity, unsigned long long& acc) {
+    if (mbar_test(bar, parity)) return;
+    const long long t0 = clock64();
+    mbar_wait(bar, parity);
+    acc += static_cast<unsigned long long>(clock64() - t0);
+}
+
+__device__ __forceinline__ void st_cg_f32(float* p, float v) {
+    asm volatile("st.global.cg.f32 [%0], %1;" ::"l"(p), "f"(v) : "memory");
+}
+
+// Store 16 token columns (rows m_first .. m_first+15 of `out`) of this lane's output feature n as
+// bf16 (RNE).  Adjacent lanes hold adjacent n: lane pairs exchange one value per two columns so
+// that every lane stores a packed bf16x2 (even lanes the even column, odd lanes the odd one).
+__device__ __forceinline__ void store_out16(__nv_bfloat16* out, size_t ld, int n, bool n_ok, int m_first, int m_end,
+                                            const float (&f)[16]) {
+    const bool odd = (threadIdx.x & 1) != 0;
+#pragma unroll
+    for (int j = 0; j < 16; j += 2) {
+        const uint32_t a = __bfloat16_as_ushort(__float2bfloat16_rn(f[j]));
+        const uint32_t b = __bfloat16_as_ushort(__float2bfloat16_rn(f[j + 1]));
+        const uint32_t recv = __shfl_xor_sync(0xffffffffu, odd ? a : b, 1);
+        const int m = m_first + j + (odd ? 1 : 0);
+        const uint32_t packed = odd ? (recv | (b << 16)) : (a | (recv << 16));
+        if (n_ok && m < m_end)
+            *reinterpret_cast<uint32_t*>(out + static_cast<size_t>(m) * ld + (n & ~1)) = packed;
+    }
+}
+
 __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_constant__ KernelParams P) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -129,12 +163,13 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
     constexpr int kBarBytes = 8 * (2 * kMaxStages + 4 + 3 * kSchedSlots);
     UnitInfo* ring = reinterpret_cast<UnitInfo*>(ctrl + kBarBytes);
     volatile uint32_t* s_tmem = reinterpret_cast<volatile uint32_t*>(ctrl + kBarBytes + sizeof(UnitInfo) * kSchedSlots);
-    volatile uint32_t* s_last = s_tmem + 1;
     volatile unsigned long long* s_epoch = reinterpret_cast<volatile unsigned long long*>(s_tmem + 2);
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
     const long long t_start = clock64();
+    CtaStats* const my_stats = P.stats + blockIdx.x;
+    if (threadIdx.x == 0) my_stats->ts[0] = globaltimer_ns();
 
     uint32_t tmem_cols = 32;
     while (tmem_cols < static_cast<uint32_t>(2 * tile_m)) tmem_cols <<= 1;
@@ -173,6 +208,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
     tc_fence_after();
     const uint32_t tmem_base = *s_tmem;
     const unsigned long long epoch = *s_epoch;
+    if (threadIdx.x == 0) my_stats->ts[1] = globaltimer_ns();
 
     // ------------------------------------------------------------------ roles
     if (warp == 0) {
@@ -181,7 +217,14 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
             uint32_t done[kMaxLayers];
             for (int l = 0; l < kMaxLayers; ++l) done[l] = 0;
             int l = P.layer_begin;
-            if (static_cast<int>(blockIdx.x) >= P.producer_ctas && P.layer_begin + 1 < P.layer_end) l = P.layer_begin + 1;
+            // the first unit of a CTA is static (its rank among the CTAs that start on the same layer):
+            // no atomic round trip before the first weight load
+            uint32_t static_id = blockIdx.x;
+            bool use_static = true;
+            if (static_cast<int>(blockIdx.x) >= P.producer_ctas && P.layer_begin + 1 < P.layer_end) {
+                l = P.layer_begin + 1;
+                static_id = blockIdx.x - P.producer_ctas;
+            }
             uint32_t it = 0;
             bool finished = false;
             while (!finished) {
@@ -192,8 +235,14 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 if (it >= 1) mbar_wait(bar_wtaken + 8 * ((it - 1) % kSchedSlots), ((it - 1) / kSchedSlots) & 1);
                 while (l < P.layer_end) {
                     const LayerParams& L = P.layer[l];
-                    const uint32_t base = static_cast<uint32_t>(epoch * static_cast<unsigned long long>(L.units + L.drawers));
-                    uint32_t t = atom_add_relaxed_gpu(L.ticket, 1u) - base;
+                    uint32_t t;
+                    if (use_static) {
+                        use_static = false;
+                        t = static_id;
+                    } else {
+                        const uint32_t base = static_cast<uint32_t>(epoch * static_cast<unsigned long long>(L.ticket_inc));
+                        t = atom_add_relaxed_gpu(L.ticket, 1u) - base + static_cast<uint32_t>(L.ticket_off);
+                    }
                     if (t >= static_cast<uint32_t>(L.units)) {
                         ++l;
                         continue;
@@ -217,6 +266,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                     u.kb0 = static_cast<int>((static_cast<long long>(ks) * L.kb_total) / L.split);
                     u.kb1 = static_cast<int>((static_cast<long long>(ks + 1) * L.kb_total) / L.split);
                     u.valid = 1;
+                    if (it == 0) my_stats->ts[2] = globaltimer_ns();
                     done[l]++;
                     break;
                 }
@@ -235,6 +285,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
             const uint64_t pol = policy_evict_first();
             const bool hint = !(P.flags & kFlagNoEvictFirst);
             uint32_t stage = 0, phase = 0;
+            unsigned long long w_wait = 0;
             for (uint32_t it = 0;; ++it) {
                 const uint32_t slot = it % kSchedSlots;
                 mbar_wait(bar_sfull + 8 * slot, (it / kSchedSlots) & 1);
@@ -244,15 +295,17 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 if (!u.valid) break;
                 const CUtensorMap* tm = &P.tm_w[u.layer];
                 for (int kb = u.kb0; kb < u.kb1; ++kb) {
-                    mbar_wait(bar_empty + 8 * stage, phase ^ 1);
+                    mbar_wait_timed(bar_empty + 8 * stage, phase ^ 1, w_wait);
                     const uint32_t full = bar_full + 8 * stage;
                     mbar_arrive_expect_tx(full, stage_bytes);
                     const uint32_t dst = smem_base + stage * stage_bytes;
                     if (hint) tma_load_2d_hint(dst, tm, kb * kTileK, u.n_blk * kTileN, full, pol);
                     else tma_load_2d(dst, tm, kb * kTileK, u.n_blk * kTileN, full);
+                    if (it == 0 && kb == u.kb0) my_stats->ts[3] = globaltimer_ns();
                     if (++stage == static_cast<uint32_t>(stages)) { stage = 0; phase ^= 1; }
                 }
             }
+            my_stats->wait[0] = w_wait;
         }
     } else if (warp == 2) {
         // ===== A loader = consumer prologue (step a5; PAPER.md:95 step (5))
@@ -314,6 +367,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
         if (lane == 0) {
             const uint32_t idesc = make_idesc_bf16(kTileN, tile_m);
             uint32_t stage = 0, phase = 0;
+            unsigned long long wait_ops = 0, wait_acc = 0;
             for (uint32_t it = 0;; ++it) {
                 const uint32_t slot = it % kSchedSlots;
                 mbar_wait(bar_sfull + 8 * slot, (it / kSchedSlots) & 1);
@@ -321,12 +375,13 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 mbar_arrive(bar_sempty + 8 * slot);
                 if (!u.valid) break;
                 const uint32_t acc = it & 1u;
-                mbar_wait(bar_tempty + 8 * acc, ((it >> 1) & 1u) ^ 1u);
+                mbar_wait_timed(bar_tempty + 8 * acc, ((it >> 1) & 1u) ^ 1u, wait_acc);
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + acc * static_cast<uint32_t>(tile_m);
                 for (int kb = u.kb0; kb < u.kb1; ++kb) {
-                    mbar_wait(bar_full + 8 * stage, phase);
+                    mbar_wait_timed(bar_full + 8 * stage, phase, wait_ops);
                     tc_fence_after();
+                    if (it == 0 && kb == u.kb0) my_stats->ts[4] = globaltimer_ns();
                     const uint32_t a_addr = smem_base + stage * stage_bytes;
                     const uint32_t b_addr = a_addr + kWTileBytes;
                     const uint64_t a_desc = make_smem_desc_sw128(a_addr);
@@ -342,11 +397,15 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 }
                 umma_commit(bar_tfull + 8 * acc);
             }
+            my_stats->wait[2] = wait_ops;
+            my_stats->wait[3] = wait_acc;
         }
     } else {
         // ===== epilogue warps 4..7 (steps a3, a4, a7, a8)
         const int r = threadIdx.x - (kThreads - kEpiThreads);  // TMEM lane = weight row inside the tile
         const int wq = r >> 5;
+        unsigned long long wait_acc = 0, wait_part = 0;
+        bool aborted = false;
         for (uint32_t it = 0;; ++it) {
             const uint32_t slot = it % kSchedSlots;
             mbar_wait(bar_sfull + 8 * slot, (it / kSchedSlots) & 1);
@@ -355,13 +414,22 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
             if (!u.valid) break;
             const LayerParams& L = P.layer[u.layer];
             const uint32_t acc = it & 1u;
-            mbar_wait(bar_tfull + 8 * acc, (it >> 1) & 1u);
+            mbar_wait_timed(bar_tfull + 8 * acc, (it >> 1) & 1u, wait_acc);
             tc_fence_after();
+            if (it == 0 && r == 0) my_stats->ts[5] = globaltimer_ns();
             const uint32_t taddr = tmem_base + (static_cast<uint32_t>(wq * 32) << 16) + acc * static_cast<uint32_t>(tile_m);
             const int n = u.n_blk * kTileN + r;
             const int m0 = P.m_off + u.m_blk * tile_m;
             const bool n_ok = n < L.N;
-            if (L.split == 1) {
+            const size_t out_row = static_cast<size_t>(L.N);
+            const size_t ks_stride = static_cast<size_t>(tile_m) * kTileN;
+            // step a8 (split-K): the slice that is ticketed LAST for its tile is the reducer; every
+            // other slice stores its fp32 partial and signals.  A unit only ever waits on units with a
+            // lower ticket, so the ticket order keeps the scheme deadlock-free.
+            const bool reversed = (P.flags & kFlagDebugReverse) && u.layer == P.layer_begin;
+            const int ks_reducer = reversed ? 0 : L.split - 1;
+            if (L.split > 1 && u.ks != ks_reducer) {
+                float* wsp = L.ws + (static_cast<size_t>(u.tile) * L.split + u.ks) * ks_stride + r;
                 for (int c0 = 0; c0 < tile_m; c0 += 16) {
                     uint32_t v[16];
                     tmem_ld16(taddr + c0, v);
@@ -370,77 +438,110 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                         tc_fence_before();
                         mbar_arrive(bar_tempty + 8 * acc);
                     }
-                    if (n_ok) {
 #pragma unroll
-                        for (int j = 0; j < 16; ++j) {
-                            const int m = m0 + c0 + j;
-                            if (m < P.m_end)
-                                L.out[static_cast<size_t>(m) * L.N + n] =
-                                    __float2bfloat16_rn(act_apply(__uint_as_float(v[j]), L.act));
+                    for (int j = 0; j < 16; ++j) st_cg_f32(wsp + static_cast<size_t>(c0 + j) * kTileN, __uint_as_float(v[j]));
+                }
+                // the 128 threads' partial stores happen-before thread 0's release (bar.sync) and a
+                // release is cumulative: one fire-and-forget red publishes the CTA's whole partial
+                bar_sync(1, kEpiThreads);
+                if (r == 0) red_release_gpu_add(L.arrive + u.tile, 1u);
+                continue;
+            }
+            if (L.split > 1) {
+                // reducer: wait for the other split-1 partials (all from lower tickets)
+                if (r == 0 && !aborted) {
+                    const uint32_t target = static_cast<uint32_t>((epoch + 1ull) * static_cast<unsigned long long>(L.split - 1));
+                    if (static_cast<int32_t>(ld_acquire_gpu(L.arrive + u.tile) - target) < 0) {
+                        const long long c0 = clock64();
+                        const uint64_t t0 = globaltimer_ns();
+                        uint32_t np = 0;
+                        while (static_cast<int32_t>(ld_acquire_gpu(L.arrive + u.tile) - target) < 0) {
+                            __nanosleep(32);
+                            if ((++np & 255u) == 0) {
+                                if (ld_relaxed_gpu(P.status) != 0) { aborted = true; break; }
+                                if (globaltimer_ns() - t0 > P.timeout_ns) {
+                                    atomicCAS(P.status, 0u, kStatusFlagTimeout);
+                                    aborted = true;
+                                    break;
+                                }
+                            }
                         }
+                        wait_part += static_cast<unsigned long long>(clock64() - c0);
                     }
                 }
-            } else {
-                // step a8: fp32 partial to the workspace; the last arriver sums the partials in fixed
-                // slice order, so the result does not depend on which CTA arrives last
-                float* wsp = L.ws + (static_cast<size_t>(u.tile) * L.split + u.ks) * (static_cast<size_t>(tile_m) * kTileN) + r;
-                for (int c0 = 0; c0 < tile_m; c0 += 16) {
-                    uint32_t v[16];
-                    tmem_ld16(taddr + c0, v);
+                bar_sync(1, kEpiThreads);  // thread 0's acquire happens-before everyone's partial loads
+            }
+            const float* wsr = L.ws + static_cast<size_t>(u.tile) * L.split * ks_stride + r;
+            for (int c0 = 0; c0 < tile_m; c0 += 16) {
+                uint32_t v[16];
+                tmem_ld16(taddr + c0, v);
+                float s[16];
+                if (L.split > 1) {
+                    // sum in slice order ks = 0 .. split-1 (own accumulator at its own position), so the
+                    // rounding does not depend on timing; up to 48 independent loads in flight per thread
+                    bool have = false;
+                    for (int ks = 0; ks < L.split; ks += 3) {
+                        float t[3][16];
+#pragma unroll
+                        for (int q = 0; q < 3; ++q)
+                            if (ks + q < L.split && ks + q != u.ks) {
+#pragma unroll
+                                for (int j = 0; j < 16; ++j)
+                                    t[q][j] = ld_cg_f32(wsr + (ks + q) * ks_stride + static_cast<size_t>(c0 + j) * kTileN);
+                            }
+#pragma unroll
+                        for (int q = 0; q < 3; ++q)
+                            if (ks + q < L.split) {
+                                if (ks + q == u.ks) {
+                                    tmem_ld_wait();
+#pragma unroll
+                                    for (int j = 0; j < 16; ++j) t[q][j] = __uint_as_float(v[j]);
+                                }
+                                if (!have) {
+#pragma unroll
+                                    for (int j = 0; j < 16; ++j) s[j] = t[q][j];
+                                    have = true;
+                                } else {
+#pragma unroll
+                                    for (int j = 0; j < 16; ++j) s[j] += t[q][j];
+                                }
+                            }
+                    }
+                } else {
                     tmem_ld_wait();
-                    if (c0 + 16 >= tile_m) {
-                        tc_fence_before();
-                        mbar_arrive(bar_tempty + 8 * acc);
-                    }
 #pragma unroll
-                    for (int j = 0; j < 16; ++j) wsp[static_cast<size_t>(c0 + j) * kTileN] = __uint_as_float(v[j]);
+                    for (int j = 0; j < 16; ++j) s[j] = __uint_as_float(v[j]);
                 }
-                __threadfence();
-                bar_sync(1, kEpiThreads);
-                if (r == 0) {
-                    const uint32_t base = static_cast<uint32_t>(epoch * static_cast<unsigned long long>(L.split));
-                    const uint32_t old = atom_add_acq_rel_gpu(L.arrive + u.tile, 1u) - base;
-                    *s_last = (old == static_cast<uint32_t>(L.split - 1)) ? 1u : 0u;
+                if (c0 + 16 >= tile_m) {  // accumulator fully read: hand TMEM back to the MMA warp
+                    tc_fence_before();
+                    mbar_arrive(bar_tempty + 8 * acc);
                 }
-                bar_sync(1, kEpiThreads);
-                const bool last = (*s_last != 0);
-                bar_sync(1, kEpiThreads);  // s_last may be rewritten by the next unit only after all have read it
-                if (!last) continue;
-                __threadfence();
-                const float* wsr = L.ws + static_cast<size_t>(u.tile) * L.split * (static_cast<size_t>(tile_m) * kTileN) + r;
-                const size_t ks_stride = static_cast<size_t>(tile_m) * kTileN;
-                for (int c0 = 0; c0 < tile_m; c0 += 8) {
-                    float s[8];
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) s[j] = ld_cg_f32(wsr + static_cast<size_t>(c0 + j) * kTileN);
-                    for (int ks = 1; ks < L.split; ++ks) {
-#pragma unroll
-                        for (int j = 0; j < 8; ++j)
-                            s[j] += ld_cg_f32(wsr + ks * ks_stride + static_cast<size_t>(c0 + j) * kTileN);
-                    }
-                    if (n_ok) {
-#pragma unroll
-                        for (int j = 0; j < 8; ++j) {
-                            const int m = m0 + c0 + j;
-                            if (m < P.m_end)
-                                L.out[static_cast<size_t>(m) * L.N + n] = __float2bfloat16_rn(act_apply(s[j], L.act));
-                        }
-                    }
-                }
+                for (int j = 0; j < 16; ++j) s[j] = act_apply(s[j], L.act);
+                store_out16(L.out, out_row, n, n_ok, m0 + c0, P.m_end, s);
             }
             if (L.publish) {
                 // producer epilogue (step a4; output tile, then fence, then the dependency
-                // update -- "only the warp responsible for writing global output issues the threadfence",
-                // PAPER.md:129; here all four epilogue warps write, so all fence, then one thread signals)
-                __threadfence();
-                fence_proxy_async();
+                // update).  All four epilogue warps wrote the tile: their stores happen-before the
+                // barrier, and thread 0's gpu-scope release after it is cumulative (the pattern of a
+                // cooperative grid barrier), so one fence + one red publishes the tile -- cf. PAPER.md:129
+                // "only the warp responsible for writing global output issues the threadfence".
+                fence_proxy_async();  // generic-proxy stores of H vs. the consumers' async-proxy (TMA) reads
                 if ((P.flags & kFlagDebugDelay) && u.layer == P.layer_begin) {
                     const uint32_t hsh = (static_cast<uint32_t>(u.tile) * 2654435761u) >> 20;  // 0..4095
                     __nanosleep((hsh & 1023u) * 16u);
                 }
                 bar_sync(1, kEpiThreads);
-                if (r == 0) red_release_gpu_add(L.ready + u.tile, 1u);
+                if (r == 0) {
+                    fence_acq_rel_gpu();
+                    red_release_gpu_add(L.ready + u.tile, 1u);
+                }
             }
+            if (it == 0 && r == 0) my_stats->ts[6] = globaltimer_ns();
+        }
+        if (r == 0) {
+            my_stats->wait[4] = wait_acc;
+            my_stats->wait[5] = wait_part;
         }
     }
 
@@ -452,7 +553,8 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
         tmem_dealloc(tmem_base, tmem_cols);
     }
     if (threadIdx.x == 0) {
-        P.stats[blockIdx.x].cycles = static_cast<unsigned long long>(clock64() - t_start);
+        my_stats->cycles = static_cast<unsigned long long>(clock64() - t_start);
+        my_stats->ts[7] = globaltimer_ns();
         atomicAdd(P.epoch_counter, 1ull);
     }
 }

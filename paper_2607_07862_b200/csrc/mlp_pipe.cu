@@ -192,7 +192,6 @@ int build_base_params(mlp_pipe* h) {
         Lp.n_blks = ceil_div(Lp.N, kTileN);
         Lp.split = h->split[l];
         Lp.units = h->tiles[l] * h->split[l];
-        Lp.drawers = h->grid;
         Lp.act = l < h->L - 1 ? h->act : kActNone;
         Lp.publish = l < h->L - 1 ? 1 : 0;
         Lp.out = l < h->L - 1 ? h->H[l] : nullptr;  // last layer: caller's Y, patched per run
@@ -241,7 +240,20 @@ int lookup_tmap(mlp_pipe* h, TmapCacheEntry* cache, int* next, const void* ptr, 
     return MLP_OK;
 }
 
-int launch(mlp_pipe* h, const KernelParams& P, cudaStream_t s) {
+// Ticket bookkeeping of one launch over layers [layer_begin, layer_end) (see kernel.cuh, scheduler):
+// CTAs that START on a layer take unit `rank` statically, everyone else draws atomically.
+void set_ticket_params(const mlp_pipe* h, KernelParams& P) {
+    const int b = P.layer_begin, e = P.layer_end, G = h->grid, p = P.producer_ctas;
+    for (int l = b; l < e; ++l) {
+        const int statics = l == b ? p : (l == b + 1 ? G - p : 0);
+        const int arrivals = l == b ? 0 : (l == b + 1 ? p : G);
+        P.layer[l].ticket_off = std::min(statics, P.layer[l].units);
+        P.layer[l].ticket_inc = P.layer[l].units + arrivals;
+    }
+}
+
+int launch(mlp_pipe* h, KernelParams& P, cudaStream_t s) {
+    set_ticket_params(h, P);
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(h->grid);
     cfg.blockDim = dim3(kThreads);
@@ -375,7 +387,6 @@ int run_impl(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStre
         P.m_end = h->M;
         P.wait_flags = 1;
         P.producer_ctas = h->producer_ctas;
-        P.layer[0].drawers = h->producer_ctas;
         P.epoch_counter = h->epoch;
         P.stats = h->stats;
         if ((rc = launch(h, P, s))) return rc;
@@ -533,13 +544,13 @@ int mlp_pipe_stats(mlp_pipe* h, mlp_stats* out, size_t bytes) {
     bool ok = st.status == 0;
     for (int l = 0; l < h->L && ok; ++l) {
         const unsigned long long e = (h->mode.kind == MLP_CTA_PIPELINED ? ep[0] : ep[l]) / h->grid;
-        const int drawers = (h->mode.kind == MLP_CTA_PIPELINED && l == 0) ? h->producer_ctas : h->grid;
+        const int arrivals = h->mode.kind != MLP_CTA_PIPELINED || l == 0 ? 0 : (l == 1 ? h->producer_ctas : h->grid);
         const uint32_t* tk = cw.data() + (h->ticket[l] - h->counters);
         const uint32_t* ar = cw.data() + (h->arrive[l] - h->counters);
         const uint32_t* rd = cw.data() + (h->ready[l] - h->counters);
-        ok = ok && tk[0] == static_cast<uint32_t>(e * static_cast<unsigned long long>(st.units[l] + drawers));
+        ok = ok && tk[0] == static_cast<uint32_t>(e * static_cast<unsigned long long>(st.units[l] + arrivals));
         for (int t = 0; t < h->tiles[l] && ok; ++t) {
-            ok = ok && ar[t] == (h->split[l] > 1 ? static_cast<uint32_t>(e * h->split[l]) : 0u);
+            ok = ok && ar[t] == static_cast<uint32_t>(e * (h->split[l] - 1));
             ok = ok && rd[t] == (l < h->L - 1 ? static_cast<uint32_t>(e) : 0u);
         }
     }
@@ -549,6 +560,18 @@ int mlp_pipe_stats(mlp_pipe* h, mlp_stats* out, size_t bytes) {
         h->poisoned_state = true;
         return fail(h, MLP_ERR_TIMEOUT, "flag-poll watchdog expired on the device (status %u)", st.status);
     }
+    return MLP_OK;
+}
+
+int mlp_pipe_cta_records(mlp_pipe* h, int cls, mlp_cta_record* out, int max_records, int* n_out) {
+    static_assert(sizeof(mlp_cta_record) == sizeof(CtaStats), "mlp_cta_record must mirror CtaStats");
+    if (!h || !out || !n_out || max_records < 0) return MLP_ERR_INVALID;
+    const int classes = h->mode.kind == MLP_CTA_PIPELINED ? 1 : h->L;
+    if (cls < 0 || cls >= classes) return fail(h, MLP_ERR_INVALID, "bad launch class %d", cls);
+    CUDA_TRY(h, cudaDeviceSynchronize());
+    const int n = std::min(max_records, h->grid);
+    CUDA_TRY(h, cudaMemcpy(out, h->stats + static_cast<size_t>(cls) * h->grid, sizeof(CtaStats) * n, cudaMemcpyDeviceToHost));
+    *n_out = n;
     return MLP_OK;
 }
 
