@@ -1,0 +1,361 @@
+#!/usr/bin/env python
+"""bench.py -- latency of the CTA-pipelined 2-layer MLP GEMM on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config I] [--mode ...]
+
+A "step" is one pass of the whole hot path (all SURVEY.md 8(a) rows: ticketing, GEMM1, activation,
+publish, poll, GEMM2, store) over one batch of synthetic input.  Workload at N = 1: BASELINE.json
+configs[1] (Llama-3-8B-shaped MLP, M = 16, 4096 -> 14336 -> 4096, GeLU(tanh), bf16).  Prints ONE JSON line.
+Multi-GPU: the path does not shard ("replicas only"): every rank runs an independent replica,
+the reported latency is the max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "mlp_2layer_gemm_latency_us"
+UNIT = "us"
+N_WEIGHT_SETS = 3  # rotating weight sets: no step can reuse the previous step's weights from L2
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (bench line: 1)")
+    ap.add_argument("--mode", default="pipelined", choices=["pipelined", "sequential", "microbatch"])
+    ap.add_argument("--chunks", type=int, default=2)
+    ap.add_argument("--sm-split", type=float, default=1.0)
+    ap.add_argument("--stages", type=int, default=0)
+    ap.add_argument("--split-k", type=str, default="", help="comma list, per layer")
+    ap.add_argument("--no-extras", action="store_true", help="skip the side measurements (other modes, e2e, cpu baseline)")
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    return ap.parse_args()
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            mp = json.load(f)
+        return float(mp["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)", mp
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)", {}
+
+
+def committed_traffic(workload: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture, or None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            return json.load(f).get(workload)
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """SM clock and throttle reasons DURING the timed region, polled through NVML in a thread (the timed
+    region is only milliseconds long, too short for `nvidia-smi -lms`); same fields as the recipe's
+    nvidia-smi clocks line in B200_PROFILING.md."""
+
+    def __init__(self, device_index: int):
+        self.idx = device_index
+        self.samples, self.reasons = [], set()
+        self.max_mhz = None
+        self._stop = False
+        self._thr = None
+        self._h = None
+
+    def start(self):
+        try:
+            import threading
+
+            import pynvml as nv
+            nv.nvmlInit()
+            self._nv = nv
+            self._h = nv.nvmlDeviceGetHandleByIndex(self.idx)
+            self.max_mhz = float(nv.nvmlDeviceGetMaxClockInfo(self._h, nv.NVML_CLOCK_SM))
+            self._thr = threading.Thread(target=self._loop, daemon=True)
+            self._thr.start()
+        except Exception:
+            self._h = None
+
+    def _loop(self):
+        nv = self._nv
+        names = {"hw_slowdown": getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8),
+                 "hw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40),
+                 "sw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20),
+                 "sw_power_cap": getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4)}
+        while not self._stop:
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self._h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(0.001)
+
+    def stop(self):
+        self._stop = True
+        if self._thr is not None:
+            self._thr.join(timeout=2)
+        out = {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+        if self.samples:
+            out["sm_mhz"] = statistics.median(self.samples)
+        return out
+
+
+def nvml_index_for(torch, dev: int) -> int:
+    """NVML index of CUDA device `dev` (they differ under CUDA_VISIBLE_DEVICES)."""
+    try:
+        import pynvml as nv
+        nv.nvmlInit()
+        uuid = "GPU-" + str(torch.cuda.get_device_properties(dev).uuid)
+        return nv.nvmlDeviceGetIndex(nv.nvmlDeviceGetHandleByUUID(uuid.encode() if isinstance(uuid, str) else uuid))
+    except Exception:
+        vis = os.environ.get("CUDA_VISIBLE_DEVICES", "")
+        try:
+            return int(vis.split(",")[dev]) if vis else dev
+        except Exception:
+            return dev
+
+
+def make_mode(B, args, n_layers):
+    kind = {"pipelined": B.MLP_CTA_PIPELINED, "sequential": B.MLP_SEQUENTIAL, "microbatch": B.MLP_MICROBATCH}[args.mode]
+    split = [int(x) for x in args.split_k.split(",")] if args.split_k else []
+    return B.make_mode(kind, chunks=args.chunks if kind == B.MLP_MICROBATCH else 0, sm_split=args.sm_split,
+                       stages=args.stages, split_k_layer=split)
+
+
+def device_inputs(torch, cfg, n_sets):
+    """Synthetic inputs created on the device with the config's distribution (DESIGN.md input recipe):
+    X ~ N(0,1) (or U[-1,1] for cfg 0), W_l ~ N(0, 1/fan_in); n_sets independent weight sets."""
+    g = torch.Generator(device="cuda")
+    g.manual_seed(cfg.seed)
+
+    def draw(shape, scale):
+        if cfg.dist == "uniform":
+            t = torch.rand(shape, device="cuda", generator=g) * 2 - 1
+        else:
+            t = torch.randn(shape, device="cuda", generator=g)
+        return (t * scale).to(torch.bfloat16)
+
+    X = draw((cfg.M, cfg.widths[0]), 1.0)
+    sets = [[draw((cfg.widths[l + 1], cfg.widths[l]), cfg.widths[l] ** -0.5) for l in range(cfg.n_layers)] for _ in range(n_sets)]
+    return X, sets
+
+
+def time_steps(torch, pipe, X, sets, Y, steps, warmup, sampler=None, dist=None):
+    """W untimed warm-up steps, then EXACTLY `steps` steps bracketed by barrier + synchronize; per-step
+    CUDA events on the launch stream give the latency distribution."""
+    n = len(sets)
+    for i in range(warmup):
+        pipe.run(X, sets[i % n], Y)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    t_all0, t_all1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    if sampler is not None:
+        sampler.start()
+    torch.cuda._sleep(2_000_000)  # ~1 ms of queue head-room so launches are not host-bound
+    t_all0.record()
+    for i in range(steps):
+        ev[i][0].record()
+        pipe.run(X, sets[(warmup + i) % n], Y)
+        ev[i][1].record()
+    t_all1.record()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    clocks = sampler.stop() if sampler is not None else None
+    per = sorted(a.elapsed_time(b) * 1e3 for a, b in ev)
+    total_ms = t_all0.elapsed_time(t_all1)
+    q = lambda f: per[min(len(per) - 1, int(f * len(per)))]
+    return {"median": q(0.5), "p10": q(0.1), "p90": q(0.9), "min": per[0], "mean": sum(per) / len(per),
+            "ms_per_step": total_ms / steps}, clocks
+
+
+def oracle_time(cfg, evaluations, rows=None):
+    """The CPU oracle as it stands, timed on this box's host cores (wall clock)."""
+    import oracle
+    from paper_2607_07862_b200 import inputs
+    X, Ws = inputs.make_inputs(cfg)
+    Xu, Wu = inputs.as_u16(X), [inputs.as_u16(w) for w in Ws]
+    if rows is not None:
+        Xu = Xu[:rows].copy()
+    ts = []
+    for _ in range(evaluations):
+        t0 = time.perf_counter()
+        oracle.mlp_chain(Xu, Wu, cfg.act)
+        ts.append((time.perf_counter() - t0) * 1e6)
+    return ts, oracle.num_threads()
+
+
+def run_reference(args):
+    """--impl reference: the oracle (kind = "oracle") on the host cores, same metric / config / unit."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from paper_2607_07862_b200 import inputs
+    cfg = inputs.CONFIGS[args.config]
+    probe, cores = oracle_time(cfg, 1)
+    rows = cfg.M
+    budget_us = 200e6
+    while rows > 1 and probe[0] * (rows / cfg.M) ** 0.5 * (args.steps + args.warmup) > budget_us:
+        rows = max(1, rows // 4)
+    ts, cores = oracle_time(cfg, args.warmup + args.steps, rows=rows if rows < cfg.M else None)
+    ts = sorted(ts[args.warmup:])
+    scale = cfg.M / rows
+    med = ts[len(ts) // 2] * scale
+    sample = (f"full workload ({cfg.M} rows) per step" if rows == cfg.M else
+              f"{rows} of {cfg.M} token rows per step, time scaled by {scale:g} (weights are converted once per step)")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": med, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": sum(ts) / len(ts) * scale / 1e3, "higher_is_better": False, "scaling": "weak",
+        "vs_baseline": None, "dtype": "bf16 in/out, fp32 accumulate", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{args.config}]: {cfg.name} M={cfg.M} widths={list(cfg.widths)}"},
+        "cpu_baseline": {"value": med, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": med, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    from paper_2607_07862_b200 import binding as B
+    from paper_2607_07862_b200 import inputs
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (sm_100a); there is no CPU fallback")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        dist_mod.init_process_group("nccl", device_id=torch.device("cuda", local))
+        dist = dist_mod
+
+    cfg = inputs.CONFIGS[args.config]
+    mode = make_mode(B, args, cfg.n_layers)
+    X, sets = device_inputs(torch, cfg, N_WEIGHT_SETS)
+    Y = torch.empty((cfg.M, cfg.widths[-1]), dtype=torch.bfloat16, device="cuda")
+    pipe = B.MlpPipe(cfg.M, cfg.widths, cfg.act, mode)
+    sampler = ClockSampler(nvml_index_for(torch, local))
+    lat, clocks = time_steps(torch, pipe, X, sets, Y, args.steps, args.warmup, sampler, dist)
+    st = pipe.stats()
+    launches_per_step = 1 if args.mode == "pipelined" else cfg.n_layers * (args.chunks if args.mode == "microbatch" else 1)
+
+    value = lat["median"]
+    ms_per_step = lat["ms_per_step"]
+    if dist is not None:  # replicas only: the job's latency is the slowest replica's
+        t = torch.tensor([value, ms_per_step], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        value, ms_per_step = float(t[0]), float(t[1])
+
+    peak, peak_src, mp = measured_peaks()
+    alg_bytes = cfg.algorithmic_bytes
+    # dominant kernel = mlp_pipe_kernel; in pipelined mode one launch per step, so its average launch
+    # duration over the timed region is the per-step event time
+    kern_us = lat["mean"] / launches_per_step if args.mode != "pipelined" else lat["mean"]
+    bytes_per_launch = alg_bytes / launches_per_step
+    achieved = bytes_per_launch / kern_us / 1e3  # GB/s
+    workload = f"cfg{args.config}_{args.mode}"
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": committed_traffic(workload), "peak_source": peak_src, "kernel": "mlp_pipe_kernel",
+                "algorithmic_bytes_per_launch": bytes_per_launch, "avg_launch_us": kern_us,
+                "roofline_us_at_peak": alg_bytes / peak / 1e3, "tflops": cfg.flops / value / 1e6}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16 in/out, fp32 accumulate", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{args.config}]: {cfg.name} M={cfg.M} widths={list(cfg.widths)} act={cfg.act}",
+                   "mode": args.mode, "grid": st.grid, "tile_m": st.tile_m, "stages": st.stages,
+                   "split_k": list(st.split_k)[:cfg.n_layers], "sm_split": args.sm_split,
+                   "l2": f"inputs larger than L2: {N_WEIGHT_SETS} rotating weight sets of {alg_bytes / 1e6:.0f} MB, no weight reuse across steps",
+                   "multi_gpu": "replicas only"},
+        "latency_us": lat, "clocks": clocks, "gpu_launches": args.steps * launches_per_step, "roofline": roofline,
+        "flag_stall_cycles_max": int(st.flag_stall_cycles_max),
+    }
+    if rank == 0 and not args.no_extras:
+        line.update(extras(torch, B, inputs, cfg, args, X, sets, Y, with_cpu=(world == 1)))
+    if dist is not None:
+        dist.barrier()
+    pipe.close()
+    if rank == 0:
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def extras(torch, B, inputs, cfg, args, X, sets, Y, with_cpu=True):
+    """Side measurements beside the headline: the in-build SEQUENTIAL and MICROBATCH modes on the same
+    inputs, the end-to-end number through the host-buffer entry point, and the timed CPU oracle."""
+    out = {}
+    modes = {}
+    for name, mode in (("sequential", B.make_mode(B.MLP_SEQUENTIAL, stages=args.stages)),
+                       ("microbatch2", B.make_mode(B.MLP_MICROBATCH, chunks=2, stages=args.stages)),
+                       ("pipelined_sm_split_0.5", B.make_mode(B.MLP_CTA_PIPELINED, sm_split=0.5, stages=args.stages))):
+        if cfg.M % 2 and name == "microbatch2":
+            continue
+        p = B.MlpPipe(cfg.M, cfg.widths, cfg.act, mode)
+        lat, _ = time_steps(torch, p, X, sets, Y, min(args.steps, 100), max(3, min(args.warmup, 10)))
+        modes[name] = {"median_us": lat["median"], "p10_us": lat["p10"], "p90_us": lat["p90"]}
+        p.close()
+    out["other_modes"] = modes
+
+    # e2e: the same step through mlp_pipe_run_host -- pinned host X / W_l in, Y out, copies inside the timed region
+    p = B.MlpPipe(cfg.M, cfg.widths, cfg.act, make_mode(B, args, cfg.n_layers))
+    Xh = X.cpu().pin_memory()
+    Wh = [w.cpu().pin_memory() for w in sets[0]]
+    Yh = torch.empty((cfg.M, cfg.widths[-1]), dtype=torch.bfloat16).pin_memory()
+    h2d = d2h = 0
+    for _ in range(3):
+        p.run_host(Xh, Wh, Yh)
+    ts = []
+    for _ in range(max(1, args.e2e_steps)):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        h2d, d2h = p.run_host(Xh, Wh, Yh)   # returns after the device->host copy of Y has completed
+        ts.append((time.perf_counter() - t0) * 1e6)
+    p.close()
+    ts.sort()
+    out["e2e"] = {"value": ts[len(ts) // 2], "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                  "steps": len(ts), "api": "mlp_pipe_run_host (pinned host buffers, wall clock around the call)"}
+    if with_cpu:
+        ts, cores = oracle_time(cfg, 10)
+        ts.sort()
+        out["cpu_baseline"] = {"value": ts[len(ts) // 2], "unit": UNIT, "cores": cores, "kind": "oracle",
+                               "sample": f"full workload ({cfg.M} token rows), median of 10 evaluations"}
+    return out
+
+
+if __name__ == "__main__":
+    sys.exit(main())
