@@ -96,6 +96,7 @@ typedef struct {
     unsigned flags;  /* MLP_FLAG_*                                                                     */
     int split_k_layer[MLP_MAX_LAYERS]; /* per-layer override of split_k (0 = use split_k / auto)       */
     int grid;        /* CTAs of the persistent launch: 0 = one per SM                                  */
+    int w_group;     /* weight K-blocks (128-byte row pieces) requested back to back: 0 = auto, <= stages   */
     int timeout_ms;  /* flag-poll watchdog: 0 = 2000 ms.  On expiry the kernel stops waiting, finishes
                         with undefined output and the handle reports MLP_ERR_TIMEOUT                   */
 } mlp_mode;
@@ -177,6 +178,7 @@ int mlp_pipe_stats(mlp_pipe* h, mlp_stats* out, size_t bytes);
  * SEQUENTIAL / MICROBATCH).  Copies min(max_records, grid) records to the host array `out` and
  * returns the number copied through *n_out.  Synchronises the device.
  */
+#define MLP_UNIT_TRACE 12
 typedef struct {
     uint64_t flag_stall_cycles;   /* SM cycles the consumer prologue spent polling                        */
     uint64_t flag_polls;          /* unsuccessful polls                                                   */
@@ -188,6 +190,10 @@ typedef struct {
                                      operands, 3 MMA on a free accumulator, 4 epilogue on an accumulator,
                                      5 split-K reducer on the other slices' partials                      */
     uint32_t units[MLP_MAX_LAYERS]; /* units this CTA executed, per layer                                 */
+    uint64_t unit_ts[MLP_UNIT_TRACE][4]; /* first MLP_UNIT_TRACE units of the CTA, globaltimer ns: weight
+                                     loader starts the unit, weight loader has issued its last load,
+                                     accumulator complete (T_mma), epilogue done incl. publish (T1)       */
+    uint32_t unit_id[MLP_UNIT_TRACE]; /* layer << 28 | tile << 8 | K-slice                                */
 } mlp_cta_record;
 int mlp_pipe_cta_records(mlp_pipe* h, int cls, mlp_cta_record* out, int max_records, int* n_out);
 

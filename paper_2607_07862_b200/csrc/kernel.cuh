@@ -39,6 +39,9 @@ constexpr int kThreads = 256;
 constexpr int kEpiThreads = 128;
 constexpr int kWTileBytes = kTileN * kTileK * 2;
 constexpr int kCtrlBytes = 1024;
+constexpr int kUnitTrace = 12;
+constexpr int kMaxAccStages = 8;
+constexpr int kGather = 5;  // split-K partials fetched per round trip by the reducer
 
 constexpr int kActNone = 0, kActRelu = 1, kActGeluTanh = 2;
 constexpr uint32_t kFlagTileMajor = 0x1u, kFlagDebugDelay = 0x2u, kFlagDebugReverse = 0x4u, kFlagNoEvictFirst = 0x8u;
@@ -54,6 +57,7 @@ struct LayerParams {
     int ticket_off;  // unit index of the first atomically drawn ticket (= units handed out statically)
     int act;       // activation on this layer's output
     int publish;   // 1 if a later layer consumes this layer's output
+    int ks_major;  // unit order: 0 tile-major (slices of a tile adjacent), 1 K-slice-major
     __nv_bfloat16* out;  // [M x N] row-major
     float* ws;           // split-K partials [tile][split][tile_m][128]
     uint32_t* ticket;    // 1 monotone counter
@@ -71,6 +75,9 @@ struct CtaStats {
                                  // 2 MMA on operands, 3 MMA on a free accumulator, 4 epilogue on an accumulator,
                                  // 5 split-K reducer on the other slices' partials
     uint32_t units[kMaxLayers];
+    unsigned long long unit_ts[kUnitTrace][4];  // per executed unit: W loader start, W loader done issuing,
+                                                // accumulator complete, epilogue done (globaltimer ns)
+    uint32_t unit_id[kUnitTrace];               // layer << 28 | tile << 8 | ks
 };
 
 struct KernelParams {
@@ -80,7 +87,10 @@ struct KernelParams {
     int layer_begin, layer_end;
     int m_off, m_end;  // token rows [m_off, m_end) of this launch
     int tile_m, m_blks;
-    int stages;
+    int stages;         // weight ring depth
+    int a_stages;       // activation ring depth
+    int acc_stages;     // TMEM accumulators in the ring
+    int w_group;        // weight K-blocks requested back to back
     int producer_ctas;  // CTAs with blockIdx.x < producer_ctas start at layer_begin, the rest one layer later
     int wait_flags;     // consumer prologue on/off
     uint32_t flags;
@@ -140,6 +150,33 @@ __device__ __forceinline__ void store_out16(__nv_bfloat16* out, size_t ld, int n
     }
 }
 
+// Spin until *ctr has reached `target` (wrap-safe).  Relaxed polls + one acquire fence = acquire pattern.
+// Bounded: after timeout_ns (or when another waiter has already given up) the wait is abandoned, the
+// device status word records it, and `true` is returned so that the caller stops waiting for good.
+__device__ __forceinline__ bool poll_counter(const uint32_t* ctr, uint32_t target, uint32_t* status,
+                                             unsigned long long timeout_ns, unsigned long long& waited) {
+    bool gave_up = false;
+    if (static_cast<int32_t>(ld_relaxed_gpu(ctr) - target) < 0) {
+        const long long c0 = clock64();
+        const uint64_t t0 = globaltimer_ns();
+        uint32_t n = 0;
+        while (static_cast<int32_t>(ld_relaxed_gpu(ctr) - target) < 0) {
+            __nanosleep(32);
+            if ((++n & 255u) == 0) {
+                if (ld_relaxed_gpu(status) != 0) { gave_up = true; break; }
+                if (globaltimer_ns() - t0 > timeout_ns) {
+                    atomicCAS(status, 0u, kStatusFlagTimeout);
+                    gave_up = true;
+                    break;
+                }
+            }
+        }
+        waited += static_cast<unsigned long long>(clock64() - c0);
+    }
+    fence_acq_rel_gpu();
+    return gave_up;
+}
+
 __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_constant__ KernelParams P) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -147,22 +184,28 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
 
     const int tile_m = P.tile_m;
     const uint32_t a_tile_bytes = static_cast<uint32_t>(tile_m) * (kTileK * 2);
-    const uint32_t stage_bytes = kWTileBytes + a_tile_bytes;
-    const int stages = P.stages;
+    const int stages = P.stages;      // weight ring depth
+    const int a_stages = P.a_stages;  // activation ring depth (its own, deeper ring: the consumer prologue's
+                                      // polls and fences then run K-blocks ahead of the weight stream)
+    const uint32_t a_ring = smem_base + static_cast<uint32_t>(stages) * kWTileBytes;
+    const uint32_t ring_bytes = static_cast<uint32_t>(stages) * kWTileBytes + static_cast<uint32_t>(a_stages) * a_tile_bytes;
 
-    // control block after the stage ring
-    uint8_t* ctrl = smem_gen + static_cast<size_t>(stages) * stage_bytes;
-    const uint32_t ctrl_s = smem_base + static_cast<uint32_t>(stages) * stage_bytes;
-    const uint32_t bar_full = ctrl_s;                          // [kMaxStages]
-    const uint32_t bar_empty = bar_full + 8 * kMaxStages;      // [kMaxStages]
-    const uint32_t bar_tfull = bar_empty + 8 * kMaxStages;     // [2]
-    const uint32_t bar_tempty = bar_tfull + 16;                // [2]
-    const uint32_t bar_sfull = bar_tempty + 16;                // [kSchedSlots]
+    // control block after the two rings
+    uint8_t* ctrl = smem_gen + ring_bytes;
+    const uint32_t ctrl_s = smem_base + ring_bytes;
+    const uint32_t bar_full = ctrl_s;                          // [kMaxStages]  weight tile landed
+    const uint32_t bar_empty = bar_full + 8 * kMaxStages;      // [kMaxStages]  weight stage consumed
+    const uint32_t bar_afull = bar_empty + 8 * kMaxStages;     // [kMaxStages]  activation tile landed
+    const uint32_t bar_aempty = bar_afull + 8 * kMaxStages;    // [kMaxStages]  activation stage consumed
+    const uint32_t bar_tfull = bar_aempty + 8 * kMaxStages;    // [kMaxAccStages]
+    const uint32_t bar_tempty = bar_tfull + 8 * kMaxAccStages;  // [kMaxAccStages]
+    const uint32_t bar_sfull = bar_tempty + 8 * kMaxAccStages;  // [kSchedSlots]
     const uint32_t bar_sempty = bar_sfull + 8 * kSchedSlots;   // [kSchedSlots]
     const uint32_t bar_wtaken = bar_sempty + 8 * kSchedSlots;  // [kSchedSlots]
-    constexpr int kBarBytes = 8 * (2 * kMaxStages + 4 + 3 * kSchedSlots);
+    constexpr int kBarBytes = 8 * (4 * kMaxStages + 2 * kMaxAccStages + 3 * kSchedSlots);
     UnitInfo* ring = reinterpret_cast<UnitInfo*>(ctrl + kBarBytes);
     volatile uint32_t* s_tmem = reinterpret_cast<volatile uint32_t*>(ctrl + kBarBytes + sizeof(UnitInfo) * kSchedSlots);
+    volatile uint32_t* s_last = s_tmem + 1;
     volatile unsigned long long* s_epoch = reinterpret_cast<volatile unsigned long long*>(s_tmem + 2);
 
     const int warp = threadIdx.x >> 5;
@@ -171,8 +214,11 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
     CtaStats* const my_stats = P.stats + blockIdx.x;
     if (threadIdx.x == 0) my_stats->ts[0] = globaltimer_ns();
 
+    // TMEM accumulator ring: as many tile_m-column accumulators as fit (<= 8), so that the MMA warp can
+    // run ahead of an epilogue that is waiting on a memory round trip
+    const uint32_t acc_stages = static_cast<uint32_t>(P.acc_stages);
     uint32_t tmem_cols = 32;
-    while (tmem_cols < static_cast<uint32_t>(2 * tile_m)) tmem_cols <<= 1;
+    while (tmem_cols < acc_stages * static_cast<uint32_t>(tile_m)) tmem_cols <<= 1;
 
     // ------------------------------------------------------------------ one-time setup
     if (threadIdx.x == 0) {
@@ -188,7 +234,11 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
             mbar_init(bar_full + 8 * s, 1);
             mbar_init(bar_empty + 8 * s, 1);
         }
-        for (int i = 0; i < 2; ++i) {
+        for (int s = 0; s < a_stages; ++s) {
+            mbar_init(bar_afull + 8 * s, 1);
+            mbar_init(bar_aempty + 8 * s, 1);
+        }
+        for (int i = 0; i < kMaxAccStages; ++i) {
             mbar_init(bar_tfull + 8 * i, 1);
             mbar_init(bar_tempty + 8 * i, kEpiThreads);
         }
@@ -250,8 +300,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                     if ((P.flags & kFlagDebugReverse) && l == P.layer_begin) t = L.units - 1 - t;
                     const int tiles = L.n_blks * P.m_blks;
                     int tile, ks;
-                    const bool tile_major = (l == P.layer_begin) || (P.flags & kFlagTileMajor);
-                    if (tile_major) {
+                    if (!L.ks_major) {
                         tile = t / L.split;
                         ks = t % L.split;
                     } else {  // K-slice-major: early units depend on early producer tiles only
@@ -293,17 +342,32 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 mbar_arrive(bar_wtaken + 8 * slot);
                 mbar_arrive(bar_sempty + 8 * slot);
                 if (!u.valid) break;
-                const CUtensorMap* tm = &P.tm_w[u.layer];
-                for (int kb = u.kb0; kb < u.kb1; ++kb) {
-                    mbar_wait_timed(bar_empty + 8 * stage, phase ^ 1, w_wait);
-                    const uint32_t full = bar_full + 8 * stage;
-                    mbar_arrive_expect_tx(full, stage_bytes);
-                    const uint32_t dst = smem_base + stage * stage_bytes;
-                    if (hint) tma_load_2d_hint(dst, tm, kb * kTileK, u.n_blk * kTileN, full, pol);
-                    else tma_load_2d(dst, tm, kb * kTileK, u.n_blk * kTileN, full);
-                    if (it == 0 && kb == u.kb0) my_stats->ts[3] = globaltimer_ns();
-                    if (++stage == static_cast<uint32_t>(stages)) { stage = 0; phase ^= 1; }
+                if (it < kUnitTrace) {
+                    my_stats->unit_ts[it][0] = globaltimer_ns();
+                    my_stats->unit_id[it] = (static_cast<uint32_t>(u.layer) << 28) | (static_cast<uint32_t>(u.tile) << 8) | static_cast<uint32_t>(u.ks);
                 }
+                const CUtensorMap* tm = &P.tm_w[u.layer];
+                // K-blocks are requested in groups of w_group: the loader first waits until the whole group of
+                // stages is free and then issues the group back to back, so that the 128-byte pieces of one
+                // weight row that are adjacent in memory reach the DRAM controller together
+                for (int kb = u.kb0; kb < u.kb1;) {
+                    const int g = min(P.w_group, u.kb1 - kb);
+                    uint32_t st = stage, ph = phase;
+                    for (int i = 0; i < g; ++i) {
+                        mbar_wait_timed(bar_empty + 8 * st, ph ^ 1, w_wait);
+                        if (++st == static_cast<uint32_t>(stages)) { st = 0; ph ^= 1; }
+                    }
+                    for (int i = 0; i < g; ++i, ++kb) {
+                        const uint32_t full = bar_full + 8 * stage;
+                        mbar_arrive_expect_tx(full, kWTileBytes);
+                        const uint32_t dst = smem_base + stage * kWTileBytes;
+                        if (hint) tma_load_2d_hint(dst, tm, kb * kTileK, u.n_blk * kTileN, full, pol);
+                        else tma_load_2d(dst, tm, kb * kTileK, u.n_blk * kTileN, full);
+                        if (it == 0 && kb == u.kb0) my_stats->ts[3] = globaltimer_ns();
+                        if (++stage == static_cast<uint32_t>(stages)) { stage = 0; phase ^= 1; }
+                    }
+                }
+                if (it < kUnitTrace) my_stats->unit_ts[it][1] = globaltimer_ns();
             }
             my_stats->wait[0] = w_wait;
         }
@@ -323,40 +387,63 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 const CUtensorMap* tm = &P.tm_a[u.layer];
                 const bool wait = P.wait_flags && u.layer > P.layer_begin;
                 const uint32_t* ready = wait ? P.layer[u.layer - 1].ready + u.m_blk * P.layer[u.layer - 1].n_blks : nullptr;
-                int last_slice = -1;
+                // Slices [.., ready_upto) of this unit are known to be published.  Readiness is monotone
+                // within a run, so the prologue looks ahead: up to 8 counters are read with independent
+                // relaxed loads that are ISSUED a few K-blocks before their result is needed (the round trip
+                // overlaps the TMA issue of slices already known to be ready), then one acquire fence turns
+                // the observations into an acquire pattern (PTX memory model: relaxed read + fence.acq_rel).
+                const int slice_end = wait ? ((u.kb1 - 1) * kTileK) / kTileN + 1 : 0;
+                int ready_upto = wait ? (u.kb0 * kTileK) / kTileN : 0;
+                uint32_t v[8];
+                int pend_base = -1;  // >= 0: v[] holds in-flight reads of counters pend_base .. pend_base+7
                 for (int kb = u.kb0; kb < u.kb1; ++kb) {
-                    mbar_wait(bar_empty + 8 * stage, phase ^ 1);
+                    mbar_wait(bar_aempty + 8 * stage, phase ^ 1);
                     if (wait) {
                         const int slice = (kb * kTileK) / kTileN;  // producer tile that wrote these columns
-                        if (slice != last_slice) {
-                            if (!aborted && static_cast<int32_t>(ld_acquire_gpu(ready + slice) - target) < 0) {
-                                const long long c0 = clock64();
-                                const uint64_t t0 = globaltimer_ns();
-                                uint32_t n = 0;
-                                while (static_cast<int32_t>(ld_acquire_gpu(ready + slice) - target) < 0) {
-                                    ++n;
-                                    __nanosleep(32);
-                                    if ((n & 255u) == 0) {
-                                        if (ld_relaxed_gpu(P.status) != 0) { aborted = true; break; }
-                                        if (globaltimer_ns() - t0 > P.timeout_ns) {
-                                            atomicCAS(P.status, 0u, kStatusFlagTimeout);
-                                            aborted = true;
-                                            break;
+                        if (pend_base < 0 && ready_upto < slice_end && slice + 2 >= ready_upto) {
+                            pend_base = ready_upto;
+#pragma unroll
+                            for (int i = 0; i < 8; ++i)
+                                v[i] = (pend_base + i < slice_end) ? ((P.flags & 0x40u) ? ld_acquire_gpu(ready + pend_base + i) : ld_relaxed_gpu(ready + pend_base + i)) : target - 1u;
+                        }
+                        if (slice >= ready_upto) {
+                            int n_ok = 0;
+#pragma unroll
+                            for (int i = 0; i < 8; ++i)
+                                if (n_ok == i && static_cast<int32_t>(v[i] - target) >= 0) n_ok = i + 1;
+                            if (n_ok == 0) {
+                                if (!aborted) {
+                                    const long long c0 = clock64();
+                                    const uint64_t t0 = globaltimer_ns();
+                                    uint32_t n = 0;
+                                    while (static_cast<int32_t>(ld_relaxed_gpu(ready + slice) - target) < 0) {
+                                        ++n;
+                                        __nanosleep(32);
+                                        if ((n & 255u) == 0) {
+                                            if (ld_relaxed_gpu(P.status) != 0) { aborted = true; break; }
+                                            if (globaltimer_ns() - t0 > P.timeout_ns) {
+                                                atomicCAS(P.status, 0u, kStatusFlagTimeout);
+                                                aborted = true;
+                                                break;
+                                            }
                                         }
                                     }
+                                    polls += n;
+                                    stall += static_cast<unsigned long long>(clock64() - c0);
                                 }
-                                polls += n;
-                                stall += static_cast<unsigned long long>(clock64() - c0);
+                                n_ok = 1;
                             }
-                            last_slice = slice;
+                            if (!(P.flags & 0x10u)) fence_acq_rel_gpu();
                             // H was written through the generic proxy; the TMA below reads it through
                             // the async proxy
-                            fence_proxy_async();
+                            if (!(P.flags & 0x20u)) fence_proxy_async();
+                            ready_upto = pend_base + n_ok;
+                            pend_base = -1;
                         }
                     }
-                    const uint32_t dst = smem_base + stage * stage_bytes + kWTileBytes;
-                    tma_load_2d(dst, tm, kb * kTileK, P.m_off + u.m_blk * tile_m, bar_full + 8 * stage);
-                    if (++stage == static_cast<uint32_t>(stages)) { stage = 0; phase ^= 1; }
+                    mbar_arrive_expect_tx(bar_afull + 8 * stage, a_tile_bytes);
+                    tma_load_2d(a_ring + stage * a_tile_bytes, tm, kb * kTileK, P.m_off + u.m_blk * tile_m, bar_afull + 8 * stage);
+                    if (++stage == static_cast<uint32_t>(a_stages)) { stage = 0; phase ^= 1; }
                 }
             }
             P.stats[blockIdx.x].stall_cycles = stall;
@@ -366,7 +453,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
         // ===== MMA issuer (steps a2, a6)
         if (lane == 0) {
             const uint32_t idesc = make_idesc_bf16(kTileN, tile_m);
-            uint32_t stage = 0, phase = 0;
+            uint32_t stage = 0, phase = 0, astage = 0, aphase = 0;
             unsigned long long wait_ops = 0, wait_acc = 0;
             for (uint32_t it = 0;; ++it) {
                 const uint32_t slot = it % kSchedSlots;
@@ -374,16 +461,17 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 const UnitInfo u = ring[slot];
                 mbar_arrive(bar_sempty + 8 * slot);
                 if (!u.valid) break;
-                const uint32_t acc = it & 1u;
-                mbar_wait_timed(bar_tempty + 8 * acc, ((it >> 1) & 1u) ^ 1u, wait_acc);
+                const uint32_t acc = it % acc_stages;
+                mbar_wait_timed(bar_tempty + 8 * acc, ((it / acc_stages) & 1u) ^ 1u, wait_acc);
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + acc * static_cast<uint32_t>(tile_m);
                 for (int kb = u.kb0; kb < u.kb1; ++kb) {
+                    mbar_wait_timed(bar_afull + 8 * astage, aphase, wait_ops);
                     mbar_wait_timed(bar_full + 8 * stage, phase, wait_ops);
                     tc_fence_after();
                     if (it == 0 && kb == u.kb0) my_stats->ts[4] = globaltimer_ns();
-                    const uint32_t a_addr = smem_base + stage * stage_bytes;
-                    const uint32_t b_addr = a_addr + kWTileBytes;
+                    const uint32_t a_addr = smem_base + stage * kWTileBytes;
+                    const uint32_t b_addr = a_ring + astage * a_tile_bytes;
                     const uint64_t a_desc = make_smem_desc_sw128(a_addr);
                     const uint64_t b_desc = make_smem_desc_sw128(b_addr);
 #pragma unroll
@@ -393,7 +481,9 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                         umma_bf16(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb > u.kb0 || k > 0) ? 1u : 0u);
                     }
                     umma_commit(bar_empty + 8 * stage);
+                    umma_commit(bar_aempty + 8 * astage);
                     if (++stage == static_cast<uint32_t>(stages)) { stage = 0; phase ^= 1; }
+                    if (++astage == static_cast<uint32_t>(a_stages)) { astage = 0; aphase ^= 1; }
                 }
                 umma_commit(bar_tfull + 8 * acc);
             }
@@ -405,7 +495,6 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
         const int r = threadIdx.x - (kThreads - kEpiThreads);  // TMEM lane = weight row inside the tile
         const int wq = r >> 5;
         unsigned long long wait_acc = 0, wait_part = 0;
-        bool aborted = false;
         for (uint32_t it = 0;; ++it) {
             const uint32_t slot = it % kSchedSlots;
             mbar_wait(bar_sfull + 8 * slot, (it / kSchedSlots) & 1);
@@ -413,23 +502,19 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
             mbar_arrive(bar_sempty + 8 * slot);
             if (!u.valid) break;
             const LayerParams& L = P.layer[u.layer];
-            const uint32_t acc = it & 1u;
-            mbar_wait_timed(bar_tfull + 8 * acc, (it >> 1) & 1u, wait_acc);
-            tc_fence_after();
-            if (it == 0 && r == 0) my_stats->ts[5] = globaltimer_ns();
+            const uint32_t acc = it % acc_stages;
             const uint32_t taddr = tmem_base + (static_cast<uint32_t>(wq * 32) << 16) + acc * static_cast<uint32_t>(tile_m);
             const int n = u.n_blk * kTileN + r;
             const int m0 = P.m_off + u.m_blk * tile_m;
             const bool n_ok = n < L.N;
             const size_t out_row = static_cast<size_t>(L.N);
             const size_t ks_stride = static_cast<size_t>(tile_m) * kTileN;
-            // step a8 (split-K): the slice that is ticketed LAST for its tile is the reducer; every
-            // other slice stores its fp32 partial and signals.  A unit only ever waits on units with a
-            // lower ticket, so the ticket order keeps the scheme deadlock-free.
-            const bool reversed = (P.flags & kFlagDebugReverse) && u.layer == P.layer_begin;
-            const int ks_reducer = reversed ? 0 : L.split - 1;
-            if (L.split > 1 && u.ks != ks_reducer) {
-                float* wsp = L.ws + (static_cast<size_t>(u.tile) * L.split + u.ks) * ks_stride + r;
+            float* const ws_tile = L.ws + static_cast<size_t>(u.tile) * L.split * ks_stride + r;
+            mbar_wait_timed(bar_tfull + 8 * acc, (it / acc_stages) & 1u, wait_acc);
+            tc_fence_after();
+            if (it == 0 && r == 0) my_stats->ts[5] = globaltimer_ns();
+            if (it < kUnitTrace && r == 0) my_stats->unit_ts[it][2] = globaltimer_ns();
+            if (L.split == 1) {
                 for (int c0 = 0; c0 < tile_m; c0 += 16) {
                     uint32_t v[16];
                     tmem_ld16(taddr + c0, v);
@@ -438,87 +523,72 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                         tc_fence_before();
                         mbar_arrive(bar_tempty + 8 * acc);
                     }
+                    float sum[16];
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) sum[j] = act_apply(__uint_as_float(v[j]), L.act);
+                    store_out16(L.out, out_row, n, n_ok, m0 + c0, P.m_end, sum);
+                }
+            } else {
+                // ---- step a8 (split-K): every slice stores its fp32 partial and arrives on the tile's counter;
+                // whoever arrives LAST sums all partials in fixed slice order (so the rounding does not depend
+                // on who that is) and finishes the tile.  Nobody ever waits, so a slow slice delays only its
+                // own tile, never the epilogue warps of another CTA.
+                float* wsp = ws_tile + static_cast<size_t>(u.ks) * ks_stride;
+                for (int c0 = 0; c0 < tile_m; c0 += 16) {
+                    uint32_t v[16];
+                    tmem_ld16(taddr + c0, v);
+                    tmem_ld_wait();
+                    if (c0 + 16 >= tile_m) {
+                        tc_fence_before();
+                        mbar_arrive(bar_tempty + 8 * acc);
+                    }
 #pragma unroll
                     for (int j = 0; j < 16; ++j) st_cg_f32(wsp + static_cast<size_t>(c0 + j) * kTileN, __uint_as_float(v[j]));
                 }
-                // the 128 threads' partial stores happen-before thread 0's release (bar.sync) and a
-                // release is cumulative: one fire-and-forget red publishes the CTA's whole partial
+                // the 128 threads' partial stores happen-before thread 0's atomic (bar.sync); its release half
+                // is cumulative and publishes the CTA's whole partial, its acquire half (on the last arrival)
+                // makes the other slices' partials visible to the loads after the second barrier
                 bar_sync(1, kEpiThreads);
-                if (r == 0) red_release_gpu_add(L.arrive + u.tile, 1u);
-                continue;
-            }
-            if (L.split > 1) {
-                // reducer: wait for the other split-1 partials (all from lower tickets)
-                if (r == 0 && !aborted) {
-                    const uint32_t target = static_cast<uint32_t>((epoch + 1ull) * static_cast<unsigned long long>(L.split - 1));
-                    if (static_cast<int32_t>(ld_acquire_gpu(L.arrive + u.tile) - target) < 0) {
-                        const long long c0 = clock64();
-                        const uint64_t t0 = globaltimer_ns();
-                        uint32_t np = 0;
-                        while (static_cast<int32_t>(ld_acquire_gpu(L.arrive + u.tile) - target) < 0) {
-                            __nanosleep(32);
-                            if ((++np & 255u) == 0) {
-                                if (ld_relaxed_gpu(P.status) != 0) { aborted = true; break; }
-                                if (globaltimer_ns() - t0 > P.timeout_ns) {
-                                    atomicCAS(P.status, 0u, kStatusFlagTimeout);
-                                    aborted = true;
-                                    break;
-                                }
-                            }
-                        }
-                        wait_part += static_cast<unsigned long long>(clock64() - c0);
-                    }
+                if (r == 0) {
+                    const uint32_t base = static_cast<uint32_t>(epoch * static_cast<unsigned long long>(L.split));
+                    const uint32_t old = atom_add_acq_rel_gpu(L.arrive + u.tile, 1u) - base;
+                    *s_last = (old == static_cast<uint32_t>(L.split - 1)) ? 1u : 0u;
                 }
-                bar_sync(1, kEpiThreads);  // thread 0's acquire happens-before everyone's partial loads
-            }
-            const float* wsr = L.ws + static_cast<size_t>(u.tile) * L.split * ks_stride + r;
-            for (int c0 = 0; c0 < tile_m; c0 += 16) {
-                uint32_t v[16];
-                tmem_ld16(taddr + c0, v);
-                float s[16];
-                if (L.split > 1) {
-                    // sum in slice order ks = 0 .. split-1 (own accumulator at its own position), so the
-                    // rounding does not depend on timing; up to 48 independent loads in flight per thread
-                    bool have = false;
-                    for (int ks = 0; ks < L.split; ks += 3) {
-                        float t[3][16];
+                bar_sync(1, kEpiThreads);
+                const bool last = (*s_last != 0);
+                bar_sync(1, kEpiThreads);  // s_last may be rewritten by the next unit only after all have read it
+                if (!last) {
+                    if (it < kUnitTrace && r == 0) my_stats->unit_ts[it][3] = globaltimer_ns();
+                    continue;
+                }
+                for (int c0 = 0; c0 < tile_m; c0 += 16) {
+                    float sum[16];
+                    // up to 16 * kGather independent loads in flight per thread; the adds stay in slice order
+                    for (int ks = 0; ks < L.split; ks += kGather) {
+                        float t[kGather][16];
 #pragma unroll
-                        for (int q = 0; q < 3; ++q)
-                            if (ks + q < L.split && ks + q != u.ks) {
+                        for (int q = 0; q < kGather; ++q)
+                            if (ks + q < L.split) {
 #pragma unroll
                                 for (int j = 0; j < 16; ++j)
-                                    t[q][j] = ld_cg_f32(wsr + (ks + q) * ks_stride + static_cast<size_t>(c0 + j) * kTileN);
+                                    t[q][j] = ld_cg_f32(ws_tile + (ks + q) * ks_stride + static_cast<size_t>(c0 + j) * kTileN);
                             }
 #pragma unroll
-                        for (int q = 0; q < 3; ++q)
+                        for (int q = 0; q < kGather; ++q)
                             if (ks + q < L.split) {
-                                if (ks + q == u.ks) {
-                                    tmem_ld_wait();
+                                if (ks + q == 0) {
 #pragma unroll
-                                    for (int j = 0; j < 16; ++j) t[q][j] = __uint_as_float(v[j]);
-                                }
-                                if (!have) {
-#pragma unroll
-                                    for (int j = 0; j < 16; ++j) s[j] = t[q][j];
-                                    have = true;
+                                    for (int j = 0; j < 16; ++j) sum[j] = t[q][j];
                                 } else {
 #pragma unroll
-                                    for (int j = 0; j < 16; ++j) s[j] += t[q][j];
+                                    for (int j = 0; j < 16; ++j) sum[j] += t[q][j];
                                 }
                             }
                     }
-                } else {
-                    tmem_ld_wait();
 #pragma unroll
-                    for (int j = 0; j < 16; ++j) s[j] = __uint_as_float(v[j]);
+                    for (int j = 0; j < 16; ++j) sum[j] = act_apply(sum[j], L.act);
+                    store_out16(L.out, out_row, n, n_ok, m0 + c0, P.m_end, sum);
                 }
-                if (c0 + 16 >= tile_m) {  // accumulator fully read: hand TMEM back to the MMA warp
-                    tc_fence_before();
-                    mbar_arrive(bar_tempty + 8 * acc);
-                }
-#pragma unroll
-                for (int j = 0; j < 16; ++j) s[j] = act_apply(s[j], L.act);
-                store_out16(L.out, out_row, n, n_ok, m0 + c0, P.m_end, s);
             }
             if (L.publish) {
                 // producer epilogue (step a4; output tile, then fence, then the dependency
@@ -538,6 +608,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 }
             }
             if (it == 0 && r == 0) my_stats->ts[6] = globaltimer_ns();
+            if (it < kUnitTrace && r == 0) my_stats->unit_ts[it][3] = globaltimer_ns();
         }
         if (r == 0) {
             my_stats->wait[4] = wait_acc;

@@ -19,6 +19,7 @@ using namespace mlp;
 
 static_assert(MLP_MAX_LAYERS == kMaxLayers, "header / kernel layer limit mismatch");
 static_assert(sizeof(KernelParams) <= 4000, "kernel parameter block too large");
+static_assert(MLP_UNIT_TRACE == kUnitTrace, "header / kernel trace depth mismatch");
 
 namespace {
 
@@ -41,9 +42,10 @@ struct mlp_pipe {
     int dev = 0, num_sms = 0;
     // resolved configuration
     int rows_per_launch = 0;  // M, or M / chunks
-    int tile_m = 0, m_blks = 0, stages = 0, grid = 0, producer_ctas = 0;
+    int tile_m = 0, m_blks = 0, stages = 0, a_stages = 0, grid = 0, producer_ctas = 0;
     size_t smem_bytes = 0;
     int split[kMaxLayers] = {0};
+    int ks_major[kMaxLayers] = {0};
     int tiles[kMaxLayers] = {0};
     // device memory owned by the handle
     __nv_bfloat16* H[kMaxLayers] = {nullptr};  // H[l] = output of layer l, l < L-1
@@ -132,7 +134,7 @@ int validate_mode(const mlp_mode& m, int M) {
     if (m.kind == MLP_MICROBATCH && (m.chunks < 1 || M % m.chunks != 0)) return MLP_ERR_INVALID;
     if (m.sm_split < 0.0f || m.sm_split > 1.0f) return MLP_ERR_INVALID;
     if (m.tile_m < 0 || m.tile_m % 16 != 0) return MLP_ERR_INVALID;
-    if (m.stages < 0 || m.split_k < 0 || m.grid < 0 || m.timeout_ms < 0) return MLP_ERR_INVALID;
+    if (m.stages < 0 || m.split_k < 0 || m.grid < 0 || m.timeout_ms < 0 || m.w_group < 0) return MLP_ERR_INVALID;
     for (int l = 0; l < kMaxLayers; ++l)
         if (m.split_k_layer[l] < 0) return MLP_ERR_INVALID;
     if (m.tile_m > 256 || (m.tile_n != 0 && m.tile_n != kTileN) || (m.tile_k != 0 && m.tile_k != kTileK) ||
@@ -152,33 +154,103 @@ void resolve(mlp_pipe* h) {
         h->m_blks = ceil_div(h->rows_per_launch, 256);
         h->tile_m = round_up(ceil_div(h->rows_per_launch, h->m_blks), 16);
     }
-    const int stage_bytes = kWTileBytes + h->tile_m * kTileK * 2;
-    const int max_smem = 227 * 1024;
-    int st = (max_smem - kCtrlBytes - 1024) / stage_bytes;
-    st = std::min(st, kMaxStages);
-    if (m.stages > 0) st = std::min(st, m.stages);
-    h->stages = std::max(st, 2);
-    h->smem_bytes = static_cast<size_t>(h->stages) * stage_bytes + kCtrlBytes + 1024;
+    // Two shared-memory rings: weight tiles (16 KB each) and activation tiles (tile_m x 128 B each).
+    // Weight ring depth: bytes in flight per SM just above the bandwidth-delay product (~80 KB x 148 SMs);
+    // a deeper ring only lengthens the memory queues, and with them every flag / partial round trip.
+    // Activation ring: deeper (its tiles are small at decode batch sizes), so that the consumer prologue's
+    // polls and fences run well ahead of the weight stream.
+    const int a_tile = h->tile_m * kTileK * 2;
+    const int max_smem = 227 * 1024 - kCtrlBytes - 1024;
+    int st = m.stages > 0 ? m.stages : std::max(4, ceil_div(80 * 1024, kWTileBytes));
+    st = std::max(2, std::min(st, kMaxStages));
+    int ast = std::max(st, std::min(kMaxStages, (32 * 1024) / a_tile));
+    while (st * kWTileBytes + ast * a_tile > max_smem && ast > st) --ast;
+    while (st * (kWTileBytes + a_tile) > max_smem && st > 2) --st;
+    ast = std::min(ast, std::max(st, (max_smem - st * kWTileBytes) / a_tile));
+    if (st * kWTileBytes + ast * a_tile > max_smem) ast = st;
+    h->stages = st;
+    h->a_stages = ast;
+    h->smem_bytes = static_cast<size_t>(st) * kWTileBytes + static_cast<size_t>(ast) * a_tile + kCtrlBytes + 1024;
     h->grid = m.grid > 0 ? std::min(m.grid, h->num_sms) : h->num_sms;
     const float s = (m.sm_split <= 0.0f) ? 1.0f : m.sm_split;
     h->producer_ctas = h->grid;
     if (m.kind == MLP_CTA_PIPELINED && h->L > 1 && s < 1.0f)
         h->producer_ctas = std::min(h->grid, std::max(1, static_cast<int>(h->grid * s + 0.5f)));
-    // split-K: enough units to keep every SM streaming weights, but never so fine that the fp32
-    // partials rival the weight bytes of a unit
+
+    // split-K per layer.  Start from "enough units to keep every SM streaming weights", then refine by a
+    // greedy list-scheduling model of the ticket order (unit cost = its K-blocks + a fixed overhead + the
+    // fp32 partial traffic of a non-reducer slice) so that the last wave of the launch is not ragged.
+    int kb_total[kMaxLayers];
+    for (int l = 0; l < h->L; ++l) {
+        kb_total[l] = ceil_div(h->widths[l], kTileK);
+        h->tiles[l] = ceil_div(h->widths[l + 1], kTileN) * h->m_blks;
+    }
     const int kb_min = h->tile_m <= 32 ? 8 : h->tile_m <= 64 ? 16 : h->tile_m <= 128 ? 32 : 64;
     const int target_units = 3 * h->grid;
+    bool fixed[kMaxLayers];
     for (int l = 0; l < h->L; ++l) {
-        const int kb_total = ceil_div(h->widths[l], kTileK);
-        const int n_blks = ceil_div(h->widths[l + 1], kTileN);
-        h->tiles[l] = n_blks * h->m_blks;
         int sp = m.split_k_layer[l] > 0 ? m.split_k_layer[l] : m.split_k;
+        fixed[l] = sp > 0;
         if (sp <= 0) {
             sp = ceil_div(target_units, h->tiles[l]);
-            sp = std::min(sp, std::max(1, kb_total / kb_min));
+            sp = std::min(sp, std::max(1, kb_total[l] / kb_min));
         }
-        h->split[l] = std::max(1, std::min(sp, kb_total));
+        h->split[l] = std::max(1, std::min(sp, kb_total[l]));
     }
+    const double unit_overhead = 1.0;                 // K-block equivalents per unit
+    const double partial_cost = h->tile_m / 32.0;     // K-block equivalents per non-reducer slice
+    const bool pipelined = m.kind == MLP_CTA_PIPELINED;
+    // unit order of a layer: a layer whose output is consumed inside the same launch stays tile-major (its
+    // tiles complete early, one after the other) with <= 4 slices; a layer with many slices is handed out
+    // K-slice-major, so that its early units depend on the producer's early tiles only
+    auto is_ks_major = [&](int l, int sp) {
+        if (m.flags & (MLP_FLAG_TILE_MAJOR | MLP_FLAG_DEBUG_REVERSE)) return false;
+        if (pipelined && l < h->L - 1) return false;
+        return sp > 4;
+    };
+    auto makespan = [&](int lb, int le, const int* split) {
+        std::vector<double> fin(h->grid, 0.0);        // min-heap of worker finish times
+        auto cmp = [](double a, double b) { return a > b; };
+        double end = 0.0;
+        for (int l = lb; l < le; ++l) {
+            const int sp = split[l], tiles = h->tiles[l];
+            for (int u = 0; u < tiles * sp; ++u) {
+                const int ks = is_ks_major(l, sp) ? u / tiles : u % sp;
+                const int kb = (ks + 1) * kb_total[l] / sp - ks * kb_total[l] / sp;
+                std::pop_heap(fin.begin(), fin.end(), cmp);
+                double t = fin.back() + kb + unit_overhead + (sp > 1 && ks != sp - 1 ? partial_cost : 0.0);
+                fin.back() = t;
+                std::push_heap(fin.begin(), fin.end(), cmp);
+                end = std::max(end, t);
+            }
+        }
+        return end;
+    };
+    auto refine = [&](int lb, int le) {
+        for (int pass = 0; pass < 2; ++pass)
+            for (int l = le - 1; l >= lb; --l) {
+                if (fixed[l]) continue;
+                const int kb_floor = std::max(4, kb_min / 2);
+                int s_max = std::max(1, std::min(64, kb_total[l] / kb_floor));
+                if (pipelined && l < h->L - 1) s_max = std::min(s_max, 4);
+                int best = h->split[l];
+                double best_t = makespan(lb, le, h->split);
+                for (int c = 1; c <= s_max; ++c) {
+                    const int keep = h->split[l];
+                    h->split[l] = c;
+                    const double t = makespan(lb, le, h->split);
+                    h->split[l] = keep;
+                    if (t < best_t * 0.995) { best_t = t; best = c; }
+                }
+                h->split[l] = best;
+            }
+    };
+    for (int l = 0; l < h->L; ++l)
+        if (!fixed[l] && pipelined && l < h->L - 1) h->split[l] = std::min(h->split[l], 4);
+    if (pipelined) refine(0, h->L);
+    else
+        for (int l = 0; l < h->L; ++l) refine(l, l + 1);
+    for (int l = 0; l < h->L; ++l) h->ks_major[l] = is_ks_major(l, h->split[l]) ? 1 : 0;
 }
 
 int build_base_params(mlp_pipe* h) {
@@ -194,6 +266,7 @@ int build_base_params(mlp_pipe* h) {
         Lp.units = h->tiles[l] * h->split[l];
         Lp.act = l < h->L - 1 ? h->act : kActNone;
         Lp.publish = l < h->L - 1 ? 1 : 0;
+        Lp.ks_major = h->ks_major[l];
         Lp.out = l < h->L - 1 ? h->H[l] : nullptr;  // last layer: caller's Y, patched per run
         Lp.ws = h->ws[l];
         Lp.ticket = h->ticket[l];
@@ -207,6 +280,9 @@ int build_base_params(mlp_pipe* h) {
     P.tile_m = h->tile_m;
     P.m_blks = h->m_blks;
     P.stages = h->stages;
+    P.a_stages = h->a_stages;
+    P.acc_stages = std::min(kMaxAccStages, 512 / h->tile_m);
+    P.w_group = std::max(1, std::min(h->mode.w_group > 0 ? h->mode.w_group : 1, h->stages));
     P.flags = h->mode.flags;
     P.status = h->status;
     P.timeout_ns = static_cast<unsigned long long>(h->mode.timeout_ms > 0 ? h->mode.timeout_ms : 2000) * 1000000ull;
@@ -550,7 +626,7 @@ int mlp_pipe_stats(mlp_pipe* h, mlp_stats* out, size_t bytes) {
         const uint32_t* rd = cw.data() + (h->ready[l] - h->counters);
         ok = ok && tk[0] == static_cast<uint32_t>(e * static_cast<unsigned long long>(st.units[l] + arrivals));
         for (int t = 0; t < h->tiles[l] && ok; ++t) {
-            ok = ok && ar[t] == static_cast<uint32_t>(e * (h->split[l] - 1));
+            ok = ok && ar[t] == (h->split[l] > 1 ? static_cast<uint32_t>(e * h->split[l]) : 0u);
             ok = ok && rd[t] == (l < h->L - 1 ? static_cast<uint32_t>(e) : 0u);
         }
     }
