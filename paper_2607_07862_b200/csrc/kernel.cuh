@@ -41,7 +41,7 @@ constexpr int kWTileBytes = kTileN * kTileK * 2;
 constexpr int kCtrlBytes = 1024;
 constexpr int kUnitTrace = 12;
 constexpr int kMaxAccStages = 8;
-constexpr int kGather = 5;  // split-K partials fetched per round trip by the reducer
+constexpr int kGather = 7;  // split-K partials fetched per round trip by the reducer
 
 constexpr int kActNone = 0, kActRelu = 1, kActGeluTanh = 2;
 constexpr uint32_t kFlagTileMajor = 0x1u, kFlagDebugDelay = 0x2u, kFlagDebugReverse = 0x4u, kFlagNoEvictFirst = 0x8u;
@@ -63,6 +63,7 @@ struct LayerParams {
     uint32_t* ticket;    // 1 monotone counter
     uint32_t* arrive;    // [tiles] monotone split-K arrival counters
     uint32_t* ready;     // [tiles] monotone ready counters, tile = m_blk * n_blks + n_blk
+    const uint16_t* kb_bounds;  // [split + 1] K-block boundaries of the slices (slices may taper)
 };
 
 struct CtaStats {
@@ -102,6 +103,7 @@ struct KernelParams {
 
 struct UnitInfo {
     int layer, m_blk, n_blk, ks, kb0, kb1, valid, tile;
+    int acquired, pad_[3];  // 1: the scheduler has already seen (and acquired) every ready counter of this unit
 };
 
 __device__ __forceinline__ float act_apply(float x, int act) {
@@ -280,7 +282,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
             while (!finished) {
                 UnitInfo u;
                 u.valid = 0;
-                u.layer = u.m_blk = u.n_blk = u.ks = u.kb0 = u.kb1 = u.tile = 0;
+                u.layer = u.m_blk = u.n_blk = u.ks = u.kb0 = u.kb1 = u.tile = u.acquired = 0;
                 // claim at most one unit ahead of the W loader (keeps the tail balanced)
                 if (it >= 1) mbar_wait(bar_wtaken + 8 * ((it - 1) % kSchedSlots), ((it - 1) / kSchedSlots) & 1);
                 while (l < P.layer_end) {
@@ -312,9 +314,31 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                     u.m_blk = tile / L.n_blks;
                     u.n_blk = tile % L.n_blks;
                     u.ks = ks;
-                    u.kb0 = static_cast<int>((static_cast<long long>(ks) * L.kb_total) / L.split);
-                    u.kb1 = static_cast<int>((static_cast<long long>(ks + 1) * L.kb_total) / L.split);
+                    u.kb0 = __ldg(L.kb_bounds + ks);
+                    u.kb1 = __ldg(L.kb_bounds + ks + 1);
                     u.valid = 1;
+                    if (P.wait_flags && l > P.layer_begin && !(P.flags & 0x80u)) {
+                        // Consumer prologue, fast path (the prologue lives in the scheduler
+                        // warp): one look at all ready counters under this unit's K range.  If every producer
+                        // tile is already published -- the normal case, the scheduler runs a unit ahead --
+                        // ONE acquire fence here covers the whole unit and the loaders never poll.  Otherwise
+                        // the activation loader polls slice by slice while the weight loader prefetches.
+                        const uint32_t target = static_cast<uint32_t>(epoch + 1ull);
+                        const uint32_t* rd = P.layer[l - 1].ready + u.m_blk * P.layer[l - 1].n_blks;
+                        const int s0 = (u.kb0 * kTileK) / kTileN, s1 = ((u.kb1 - 1) * kTileK) / kTileN + 1;
+                        bool all = (s1 - s0) <= 32;
+                        for (int sb = s0; sb < s1 && all; sb += 8) {
+                            uint32_t v[8];
+#pragma unroll
+                            for (int i = 0; i < 8; ++i) v[i] = (sb + i < s1) ? ld_relaxed_gpu(rd + sb + i) : target;
+#pragma unroll
+                            for (int i = 0; i < 8; ++i) all = all && static_cast<int32_t>(v[i] - target) >= 0;
+                        }
+                        if (all) {
+                            fence_acq_rel_gpu();
+                            u.acquired = 1;
+                        }
+                    }
                     if (it == 0) my_stats->ts[2] = globaltimer_ns();
                     done[l]++;
                     break;
@@ -385,7 +409,8 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 mbar_arrive(bar_sempty + 8 * slot);
                 if (!u.valid) break;
                 const CUtensorMap* tm = &P.tm_a[u.layer];
-                const bool wait = P.wait_flags && u.layer > P.layer_begin;
+                const bool wait = P.wait_flags && u.layer > P.layer_begin && !u.acquired;
+                if (P.wait_flags && u.layer > P.layer_begin) fence_proxy_async();
                 const uint32_t* ready = wait ? P.layer[u.layer - 1].ready + u.m_blk * P.layer[u.layer - 1].n_blks : nullptr;
                 // Slices [.., ready_upto) of this unit are known to be published.  Readiness is monotone
                 // within a run, so the prologue looks ahead: up to 8 counters are read with independent
@@ -602,10 +627,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                     __nanosleep((hsh & 1023u) * 16u);
                 }
                 bar_sync(1, kEpiThreads);
-                if (r == 0) {
-                    fence_acq_rel_gpu();
-                    red_release_gpu_add(L.ready + u.tile, 1u);
-                }
+                if (r == 0) red_release_gpu_add(L.ready + u.tile, 1u);  // release: orders the tile before the counter
             }
             if (it == 0 && r == 0) my_stats->ts[6] = globaltimer_ns();
             if (it < kUnitTrace && r == 0) my_stats->unit_ts[it][3] = globaltimer_ns();

@@ -46,6 +46,8 @@ struct mlp_pipe {
     size_t smem_bytes = 0;
     int split[kMaxLayers] = {0};
     int ks_major[kMaxLayers] = {0};
+    std::vector<int> bounds[kMaxLayers];       // K-block boundaries of the slices, split[l] + 1 entries
+    uint16_t* d_bounds[kMaxLayers] = {nullptr};  // the same on the device
     int tiles[kMaxLayers] = {0};
     // device memory owned by the handle
     __nv_bfloat16* H[kMaxLayers] = {nullptr};  // H[l] = output of layer l, l < L-1
@@ -177,80 +179,130 @@ void resolve(mlp_pipe* h) {
     if (m.kind == MLP_CTA_PIPELINED && h->L > 1 && s < 1.0f)
         h->producer_ctas = std::min(h->grid, std::max(1, static_cast<int>(h->grid * s + 0.5f)));
 
-    // split-K per layer.  Start from "enough units to keep every SM streaming weights", then refine by a
-    // greedy list-scheduling model of the ticket order (unit cost = its K-blocks + a fixed overhead + the
-    // fp32 partial traffic of a non-reducer slice) so that the last wave of the launch is not ragged.
+    // split-K per layer: the K-blocks of an output tile are cut into slices at h->bounds[l][0..split].
+    //  * a layer whose output is consumed inside the same launch stays tile-major (its tiles complete early,
+    //    one after the other) with <= 4 equal slices;
+    //  * a layer with more slices is handed out K-slice-major, so that its early units depend on the
+    //    producer's early tiles only; if it is the LAST layer of the launch its slices taper (guided
+    //    self-scheduling: each group of `tiles` units gets remaining_work / (2 * grid), within [4, cap]
+    //    K-blocks), so that the dynamic ticket ends the launch with small units and a short ragged tail.
+    // Candidates are ranked by a greedy list-scheduling model of the ticket order with +-8 % worker speeds.
     int kb_total[kMaxLayers];
     for (int l = 0; l < h->L; ++l) {
         kb_total[l] = ceil_div(h->widths[l], kTileK);
         h->tiles[l] = ceil_div(h->widths[l + 1], kTileN) * h->m_blks;
     }
+    const bool pipelined = m.kind == MLP_CTA_PIPELINED;
     const int kb_min = h->tile_m <= 32 ? 8 : h->tile_m <= 64 ? 16 : h->tile_m <= 128 ? 32 : 64;
-    const int target_units = 3 * h->grid;
+    const bool force_tile_major = (m.flags & (MLP_FLAG_TILE_MAJOR | MLP_FLAG_DEBUG_REVERSE)) != 0;
+    auto producer_in_launch = [&](int l) { return pipelined && l < h->L - 1; };
+    auto uniform = [&](int l, int sp) {
+        sp = std::max(1, std::min(sp, kb_total[l]));
+        std::vector<int> b(sp + 1);
+        for (int i = 0; i <= sp; ++i) b[i] = static_cast<int>(static_cast<long long>(i) * kb_total[l] / sp);
+        return b;
+    };
+    auto tapered = [&](int l, int cap) {
+        const int lo = std::max(4, kb_min / 2);
+        std::vector<int> b{0};
+        int rem = kb_total[l];
+        while (rem > 0) {
+            int sz = static_cast<int>(static_cast<long long>(rem) * h->tiles[l] / (2 * h->grid));
+            sz = std::max(lo, std::min(cap, sz));
+            if (rem - sz < lo) sz = rem;
+            b.push_back(b.back() + sz);
+            rem -= sz;
+        }
+        return b;
+    };
+    auto ks_major_of = [&](int l, const std::vector<int>& b) {
+        return !force_tile_major && !producer_in_launch(l) && b.size() - 1 > 4;
+    };
+    // Costs in K-block equivalents (one K-block streams in ~0.36 us per SM), fitted to unit traces on cfg 1:
+    // every gpu-scope fence costs the SM ~1 us of streaming, and a unit of a split tile needs one (the
+    // arrival atomic), a consumer unit another one (the acquire of its ready counters).
+    const double unit_overhead = 1.0;
+    const double fence_cost = 2.5;
+    const double partial_cost = h->tile_m / 32.0;  // fp32 partial traffic per slice of a split tile
+    const double gather_cost = 0.55;               // per slice, paid once at the end of the launch by the last tile
+    const double publish_latency = 4.0;            // K-block equivalents from the last slice's MMA to a visible tile
+    auto makespan = [&](int lb, int le) {
+        std::vector<std::pair<double, int>> fin(h->grid);  // min-heap of (finish time, worker)
+        for (int i = 0; i < h->grid; ++i) fin[i] = {0.0, i};
+        auto cmp = [](const std::pair<double, int>& x, const std::pair<double, int>& y) { return x.first > y.first; };
+        double end = 0.0;
+        std::vector<double> done_prev, done_cur;  // per output tile: when it is published
+        for (int l = lb; l < le; ++l) {
+            const std::vector<int>& b = h->bounds[l];
+            const int sp = static_cast<int>(b.size()) - 1, tiles = h->tiles[l];
+            const int n_blks = tiles / h->m_blks;
+            const int n_blks_prev = l > lb ? h->tiles[l - 1] / h->m_blks : 0;
+            const bool ksm = ks_major_of(l, b);
+            done_cur.assign(tiles, 0.0);
+            for (int u = 0; u < tiles * sp; ++u) {
+                const int ks = ksm ? u / tiles : u % sp;
+                const int tile = ksm ? u % tiles : u / sp;
+                std::pop_heap(fin.begin(), fin.end(), cmp);
+                const double speed = 1.0 + 0.08 * (((fin.back().second * 37) % 11) - 5) / 5.0;
+                double start = fin.back().first;
+                if (l > lb) {  // the consumer prologue waits for the producer tiles under its K range
+                    const int m_blk = tile / n_blks;
+                    for (int j = (b[ks] * kTileK) / kTileN; j <= ((b[ks + 1] - 1) * kTileK) / kTileN && j < n_blks_prev; ++j)
+                        start = std::max(start, done_prev[m_blk * n_blks_prev + j]);
+                }
+                const double ovh = unit_overhead + (sp > 1 ? partial_cost + fence_cost : 0.0) + (l > lb && pipelined ? fence_cost : 0.0);
+                const double t = start + (b[ks + 1] - b[ks] + ovh) * speed;
+                fin.back().first = t;
+                std::push_heap(fin.begin(), fin.end(), cmp);
+                done_cur[tile] = std::max(done_cur[tile], t + publish_latency);
+                end = std::max(end, t);
+            }
+            done_prev.swap(done_cur);
+            if (l == le - 1 && sp > 1) end += gather_cost * sp;
+        }
+        return end;
+    };
     bool fixed[kMaxLayers];
     for (int l = 0; l < h->L; ++l) {
         int sp = m.split_k_layer[l] > 0 ? m.split_k_layer[l] : m.split_k;
         fixed[l] = sp > 0;
         if (sp <= 0) {
-            sp = ceil_div(target_units, h->tiles[l]);
-            sp = std::min(sp, std::max(1, kb_total[l] / kb_min));
+            sp = std::min(ceil_div(3 * h->grid, h->tiles[l]), std::max(1, kb_total[l] / kb_min));
+            if (producer_in_launch(l)) sp = std::min(sp, 4);
         }
-        h->split[l] = std::max(1, std::min(sp, kb_total[l]));
+        h->bounds[l] = uniform(l, sp);
     }
-    const double unit_overhead = 1.0;                 // K-block equivalents per unit
-    const double partial_cost = h->tile_m / 32.0;     // K-block equivalents per non-reducer slice
-    const bool pipelined = m.kind == MLP_CTA_PIPELINED;
-    // unit order of a layer: a layer whose output is consumed inside the same launch stays tile-major (its
-    // tiles complete early, one after the other) with <= 4 slices; a layer with many slices is handed out
-    // K-slice-major, so that its early units depend on the producer's early tiles only
-    auto is_ks_major = [&](int l, int sp) {
-        if (m.flags & (MLP_FLAG_TILE_MAJOR | MLP_FLAG_DEBUG_REVERSE)) return false;
-        if (pipelined && l < h->L - 1) return false;
-        return sp > 4;
-    };
-    auto makespan = [&](int lb, int le, const int* split) {
-        std::vector<double> fin(h->grid, 0.0);        // min-heap of worker finish times
-        auto cmp = [](double a, double b) { return a > b; };
-        double end = 0.0;
-        for (int l = lb; l < le; ++l) {
-            const int sp = split[l], tiles = h->tiles[l];
-            for (int u = 0; u < tiles * sp; ++u) {
-                const int ks = is_ks_major(l, sp) ? u / tiles : u % sp;
-                const int kb = (ks + 1) * kb_total[l] / sp - ks * kb_total[l] / sp;
-                std::pop_heap(fin.begin(), fin.end(), cmp);
-                double t = fin.back() + kb + unit_overhead + (sp > 1 && ks != sp - 1 ? partial_cost : 0.0);
-                fin.back() = t;
-                std::push_heap(fin.begin(), fin.end(), cmp);
-                end = std::max(end, t);
-            }
-        }
-        return end;
-    };
     auto refine = [&](int lb, int le) {
         for (int pass = 0; pass < 2; ++pass)
             for (int l = le - 1; l >= lb; --l) {
                 if (fixed[l]) continue;
+                std::vector<std::vector<int>> cand;
                 const int kb_floor = std::max(4, kb_min / 2);
                 int s_max = std::max(1, std::min(64, kb_total[l] / kb_floor));
-                if (pipelined && l < h->L - 1) s_max = std::min(s_max, 4);
-                int best = h->split[l];
-                double best_t = makespan(lb, le, h->split);
-                for (int c = 1; c <= s_max; ++c) {
-                    const int keep = h->split[l];
-                    h->split[l] = c;
-                    const double t = makespan(lb, le, h->split);
-                    h->split[l] = keep;
+                if (producer_in_launch(l)) s_max = std::min(s_max, 4);
+                for (int c = 1; c <= s_max; ++c) cand.push_back(uniform(l, c));
+                if (l == le - 1 && !force_tile_major && !producer_in_launch(l))
+                    for (int cap : {2 * kb_floor, 3 * kb_floor, 4 * kb_floor, 6 * kb_floor, 8 * kb_floor}) {
+                        std::vector<int> t = tapered(l, cap);
+                        if (t.size() - 1 > 4 && t.size() - 1 <= 64) cand.push_back(t);
+                    }
+                std::vector<int> best = h->bounds[l];
+                double best_t = makespan(lb, le);
+                for (auto& c : cand) {
+                    h->bounds[l] = c;
+                    const double t = makespan(lb, le);
                     if (t < best_t * 0.995) { best_t = t; best = c; }
                 }
-                h->split[l] = best;
+                h->bounds[l] = best;
             }
     };
-    for (int l = 0; l < h->L; ++l)
-        if (!fixed[l] && pipelined && l < h->L - 1) h->split[l] = std::min(h->split[l], 4);
     if (pipelined) refine(0, h->L);
     else
         for (int l = 0; l < h->L; ++l) refine(l, l + 1);
-    for (int l = 0; l < h->L; ++l) h->ks_major[l] = is_ks_major(l, h->split[l]) ? 1 : 0;
+    for (int l = 0; l < h->L; ++l) {
+        h->split[l] = static_cast<int>(h->bounds[l].size()) - 1;
+        h->ks_major[l] = ks_major_of(l, h->bounds[l]) ? 1 : 0;
+    }
 }
 
 int build_base_params(mlp_pipe* h) {
@@ -267,6 +319,7 @@ int build_base_params(mlp_pipe* h) {
         Lp.act = l < h->L - 1 ? h->act : kActNone;
         Lp.publish = l < h->L - 1 ? 1 : 0;
         Lp.ks_major = h->ks_major[l];
+        Lp.kb_bounds = h->d_bounds[l];
         Lp.out = l < h->L - 1 ? h->H[l] : nullptr;  // last layer: caller's Y, patched per run
         Lp.ws = h->ws[l];
         Lp.ticket = h->ticket[l];
@@ -401,6 +454,11 @@ int create_impl(mlp_pipe** out, int M, int L, const int* widths, int dtype, int 
             h->ready[l] = p;
             p += round_up(h->tiles[l], 32);
         }
+    }
+    for (int l = 0; l < L; ++l) {
+        std::vector<uint16_t> b16(h->bounds[l].begin(), h->bounds[l].end());
+        CREATE_TRY(cudaMalloc(&h->d_bounds[l], b16.size() * sizeof(uint16_t)));
+        CREATE_TRY(cudaMemcpy(h->d_bounds[l], b16.data(), b16.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
     }
     for (int l = 0; l < L; ++l)
         if (h->split[l] > 1)
@@ -657,6 +715,7 @@ void mlp_pipe_destroy(mlp_pipe* h) {
     for (int l = 0; l < kMaxLayers; ++l) {
         if (h->H[l]) cudaFree(h->H[l]);
         if (h->ws[l]) cudaFree(h->ws[l]);
+        if (h->d_bounds[l]) cudaFree(h->d_bounds[l]);
         if (h->stage_W[l]) cudaFree(h->stage_W[l]);
     }
     if (h->counters) cudaFree(h->counters);
