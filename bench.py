@@ -193,6 +193,13 @@ def time_steps(torch, pipe, X, sets, Y, steps, warmup, sampler=None, dist=None):
             "ms_per_step": total_ms / steps}, clocks
 
 
+def max_over_ranks(torch, dist, values, device):
+    """Replicas only: a time-like metric of the job is the slowest rank's."""
+    t = torch.tensor(list(values), device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
+
+
 def oracle_time(cfg, evaluations, rows=None):
     """The CPU oracle as it stands, timed on this box's host cores (wall clock)."""
     import oracle
@@ -274,9 +281,7 @@ def main():
     value = lat["median"]
     ms_per_step = lat["ms_per_step"]
     if dist is not None:  # replicas only: the job's latency is the slowest replica's
-        t = torch.tensor([value, ms_per_step], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        value, ms_per_step = float(t[0]), float(t[1])
+        value, ms_per_step = max_over_ranks(torch, dist, [value, ms_per_step], "cuda")
 
     peak, peak_src, mp = measured_peaks()
     alg_bytes = cfg.algorithmic_bytes
