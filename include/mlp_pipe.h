@@ -88,7 +88,8 @@ typedef struct {
                         the others start on layer 2 at once (prefetch W_2, poll for H).  1 = the pure
                         single-ticket scheme.  0 is read as 1.                                         */
     int tile_m;      /* tokens per tile (the tcgen05 N extent): 0 = auto, else a multiple of 16 <= 256 */
-    int tile_n;      /* weight rows per tile (the tcgen05 M extent): 0 or 128                          */
+    int tile_n;      /* weight rows per unit: 0 = auto, 128, or 256 (two 128-row MMAs per K step that share
+                        the activation tile; needs 2 * tile_m <= 512 TMEM columns)                      */
     int tile_k;      /* contraction elements per pipeline stage: 0 or 64                               */
     int stages;      /* shared-memory ring depth: 0 = as many as fit                                   */
     int kslice_tiles;/* producer tiles per ready counter: 0 or 1 (one counter per (M-block, K-slice))  */
@@ -157,7 +158,8 @@ int mlp_pipe_poison_hidden(mlp_pipe* h, uint16_t pattern, void* cuda_stream);
 typedef struct {
     int n_layers, grid, stages, tile_m;           /* resolved launch configuration                    */
     int split_k[MLP_MAX_LAYERS];                  /* resolved per-layer split                         */
-    int units[MLP_MAX_LAYERS];                    /* work units per layer (tiles x split)             */
+    int units[MLP_MAX_LAYERS];                    /* tickets per layer (tiles x split MMA units + the
+                                                     reduce units of split tiles, if any)             */
     int producer_ctas;                            /* CTAs that start on layer 1 (sm_split)            */
     uint32_t status;                              /* 0 ok, else device-side abort code                */
     uint64_t runs;                                /* completed launches counted by the device epoch   */
@@ -169,6 +171,9 @@ typedef struct {
     uint32_t units_by_consumer_ctas[MLP_MAX_LAYERS]; /* of which by CTAs in the consumer-first group  */
     uint32_t ready_ok;                            /* 1 if every ready counter / ticket / arrival
                                                      counter holds its expected post-run value       */
+    int tile_n;                                   /* resolved weight rows per unit (128 or 256)       */
+    int reduce_mode[MLP_MAX_LAYERS];              /* how split tiles are summed: 0 not split, 1 by the
+                                                     last-arriving slice, 2 by reduce units           */
 } mlp_stats;
 int mlp_pipe_stats(mlp_pipe* h, mlp_stats* out, size_t bytes);
 
@@ -186,14 +191,16 @@ typedef struct {
     uint64_t ts[8];               /* globaltimer ns: 0 CTA start, 1 setup done, 2 first ticket decoded,
                                      3 first weight TMA issued, 4 first stage landed, 5 first accumulator
                                      complete, 6 first unit stored (+published), 7 CTA exit               */
-    uint64_t wait[6];             /* SM cycles blocked: 0 weight loader on a free stage, 1 unused, 2 MMA on
-                                     operands, 3 MMA on a free accumulator, 4 epilogue on an accumulator,
-                                     5 split-K reducer on the other slices' partials                      */
+    uint64_t wait[8];             /* SM cycles: 0 weight loader blocked on a free stage, 1 reducer summing
+                                     partials (gather loads + adds), 2 MMA blocked on operands, 3 MMA blocked
+                                     on a free accumulator, 4 epilogue blocked on an accumulator, 5 reduce unit
+                                     blocked on the arrival counter of its tile, 6 storing split-K partials,
+                                     7 direct epilogue (TMEM -> act -> bf16 -> global)                      */
     uint32_t units[MLP_MAX_LAYERS]; /* units this CTA executed, per layer                                 */
     uint64_t unit_ts[MLP_UNIT_TRACE][4]; /* first MLP_UNIT_TRACE units of the CTA, globaltimer ns: weight
                                      loader starts the unit, weight loader has issued its last load,
                                      accumulator complete (T_mma), epilogue done incl. publish (T1)       */
-    uint32_t unit_id[MLP_UNIT_TRACE]; /* layer << 28 | tile << 8 | K-slice                                */
+    uint32_t unit_id[MLP_UNIT_TRACE]; /* layer << 28 | tile << 8 | K-slice (reduce unit: 0x80 | first column / 16) */
 } mlp_cta_record;
 int mlp_pipe_cta_records(mlp_pipe* h, int cls, mlp_cta_record* out, int max_records, int* n_out);
 

@@ -48,13 +48,14 @@ class mlp_stats(ctypes.Structure):
         ("flag_polls", ctypes.c_uint64), ("kernel_cycles_max", ctypes.c_uint64),
         ("units_done", ctypes.c_uint32 * MLP_MAX_LAYERS),
         ("units_by_consumer_ctas", ctypes.c_uint32 * MLP_MAX_LAYERS), ("ready_ok", ctypes.c_uint32),
+        ("tile_n", ctypes.c_int), ("reduce_mode", ctypes.c_int * MLP_MAX_LAYERS),
     ]
 
 
 class mlp_cta_record(ctypes.Structure):
     _fields_ = [
         ("flag_stall_cycles", ctypes.c_uint64), ("flag_polls", ctypes.c_uint64), ("cycles", ctypes.c_uint64),
-        ("ts", ctypes.c_uint64 * 8), ("wait", ctypes.c_uint64 * 6), ("units", ctypes.c_uint32 * MLP_MAX_LAYERS),
+        ("ts", ctypes.c_uint64 * 8), ("wait", ctypes.c_uint64 * 8), ("units", ctypes.c_uint32 * MLP_MAX_LAYERS),
         ("unit_ts", (ctypes.c_uint64 * 4) * 12), ("unit_id", ctypes.c_uint32 * 12),
     ]
 
@@ -124,9 +125,10 @@ def _check(status: int, handle=None):
 
 def make_mode(kind: int = MLP_CTA_PIPELINED, chunks: int = 0, sm_split: float = 1.0, tile_m: int = 0, stages: int = 0,
               split_k: int = 0, split_k_layer: Sequence[int] = (), flags: int = 0, grid: int = 0,
-              timeout_ms: int = 0, w_group: int = 0) -> mlp_mode:
+              timeout_ms: int = 0, w_group: int = 0, tile_n: int = 0) -> mlp_mode:
     m = mlp_mode()
     m.kind, m.chunks, m.sm_split, m.tile_m, m.stages = kind, chunks, sm_split, tile_m, stages
+    m.tile_n = tile_n
     m.split_k, m.flags, m.grid, m.timeout_ms = split_k, flags, grid, timeout_ms
     m.w_group = w_group
     for i, s in enumerate(split_k_layer):

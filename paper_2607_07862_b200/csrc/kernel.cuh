@@ -8,9 +8,17 @@
 // core computes  D[n, m] = sum_k W_l[n, k] * A^{l-1}[m, k]  with
 //     A operand = W tile      128 weight rows (n) x 64 k, K-major, 128B swizzle   (16 KB)
 //     B operand = activation  tile_m tokens (m)   x 64 k, K-major, 128B swizzle   (tile_m * 128 B)
-//     D         = TMEM, lane = n (128 lanes), column = m (tile_m fp32 columns), double buffered
+//     D         = TMEM, lane = n (128 lanes), column = m (tile_m fp32 columns), a ring of accumulators
 // so that a decode-sized batch (M = 16) costs a 128 x 16 MMA instead of a padded 128 x 128 one and
-// every weight byte is loaded exactly once.
+// every weight byte is loaded exactly once.  With n_sub = 2 a unit covers 256 weight rows (two
+// 128-row MMAs per K step that share the activation tile in shared memory), which halves the
+// activation bytes pulled from L2 per weight byte -- what bounds the kernel once M >= 128.
+//
+// Work units come from a per-layer UNIT TABLE written by the host (mlp_pipe.cu: resolve): ticket t
+// of layer l is table_l[t].  Two kinds: an MMA unit (tile, K-slice [kb0, kb1)) and a REDUCE unit
+// (tile, token columns [c0, c1)) that sums the split-K partials of a tile in fixed slice order.  A
+// unit only ever depends on units with a lower ticket of its own layer (reduce after its slices) or
+// on units of the layer before.
 //
 // Warp roles (protocol hidden in the scheduler and store warps of a
 // warp-specialised persistent kernel):
@@ -42,6 +50,20 @@ constexpr int kCtrlBytes = 1024;
 constexpr int kUnitTrace = 12;
 constexpr int kMaxAccStages = 8;
 constexpr int kGather = 7;  // split-K partials fetched per round trip by the reducer
+constexpr int kStageTokens = 32;                            // tokens per epilogue staging buffer
+constexpr int kStageBufBytes = kStageTokens * kTileN * 2;   // [32 tokens][128 features] bf16
+constexpr int kStageBytes = 2 * kStageBufBytes;             // double buffered
+constexpr int kUnitMma = 0, kUnitReduce = 1;
+constexpr int kReduceNone = 0, kReduceLastArriver = 1, kReduceUnits = 2;
+
+// One entry of a layer's unit table = one ticket.
+struct UnitDesc {
+    uint16_t tile;  // m_blk * n_blks + n_blk
+    uint8_t kind;   // kUnitMma | kUnitReduce
+    uint8_t ks;     // K-slice index (MMA unit)
+    uint16_t a, b;  // MMA unit: K-blocks [a, b); reduce unit: token columns [a, b) of the tile
+};
+static_assert(sizeof(UnitDesc) == 8, "UnitDesc is read as one 8-byte word");
 
 constexpr int kActNone = 0, kActRelu = 1, kActGeluTanh = 2;
 constexpr uint32_t kFlagTileMajor = 0x1u, kFlagDebugDelay = 0x2u, kFlagDebugReverse = 0x4u, kFlagNoEvictFirst = 0x8u;
@@ -50,20 +72,21 @@ constexpr uint32_t kStatusFlagTimeout = 1u;
 struct LayerParams {
     int K, N;
     int kb_total;  // ceil(K / 64)
-    int n_blks;    // ceil(N / 128)
+    int n_blks;    // ceil(N / (128 * n_sub))
     int split;     // split of the contraction per output tile
-    int units;     // n_blks * m_blks * split
+    int units;     // entries of the unit table (MMA units + reduce units)
     int ticket_inc;  // what one launch adds to the ticket counter: units + CTAs arriving from the layer before
     int ticket_off;  // unit index of the first atomically drawn ticket (= units handed out statically)
     int act;       // activation on this layer's output
     int publish;   // 1 if a later layer consumes this layer's output
-    int ks_major;  // unit order: 0 tile-major (slices of a tile adjacent), 1 K-slice-major
+    int reduce_mode;  // kReduceNone (split == 1) | kReduceLastArriver | kReduceUnits
+    int ready_inc;    // what one run adds to a tile's ready counter (1, or its number of reduce units)
     __nv_bfloat16* out;  // [M x N] row-major
-    float* ws;           // split-K partials [tile][split][tile_m][128]
+    float* ws;           // split-K partials [tile][split][n_sub][tile_m / 4][128][4]
     uint32_t* ticket;    // 1 monotone counter
     uint32_t* arrive;    // [tiles] monotone split-K arrival counters
     uint32_t* ready;     // [tiles] monotone ready counters, tile = m_blk * n_blks + n_blk
-    const uint16_t* kb_bounds;  // [split + 1] K-block boundaries of the slices (slices may taper)
+    const UnitDesc* table;  // [units] ticket -> unit
 };
 
 struct CtaStats {
@@ -72,9 +95,10 @@ struct CtaStats {
     unsigned long long cycles;
     unsigned long long ts[8];  // globaltimer ns: 0 start, 1 setup done, 2 first ticket, 3 first W TMA issued,
                                // 4 first stage landed, 5 first accumulator ready, 6 first unit stored, 7 exit
-    unsigned long long wait[6];  // SM cycles blocked: 0 W loader on a free stage, 1 (unused, see stall_cycles),
-                                 // 2 MMA on operands, 3 MMA on a free accumulator, 4 epilogue on an accumulator,
-                                 // 5 split-K reducer on the other slices' partials
+    unsigned long long wait[8];  // SM cycles: 0 W loader blocked on a free stage, 1 reducer summing partials,
+                                 // 2 MMA blocked on operands, 3 MMA blocked on a free accumulator, 4 epilogue
+                                 // blocked on an accumulator, 5 reduce unit blocked on its tile's arrival counter,
+                                 // 6 storing split-K partials, 7 direct epilogue
     uint32_t units[kMaxLayers];
     unsigned long long unit_ts[kUnitTrace][4];  // per executed unit: W loader start, W loader done issuing,
                                                 // accumulator complete, epilogue done (globaltimer ns)
@@ -88,9 +112,11 @@ struct KernelParams {
     int layer_begin, layer_end;
     int m_off, m_end;  // token rows [m_off, m_end) of this launch
     int tile_m, m_blks;
+    int n_sub;          // 128-row MMAs per unit and K step (1 or 2): a unit covers 128 * n_sub weight rows
     int stages;         // weight ring depth
     int a_stages;       // activation ring depth
     int acc_stages;     // TMEM accumulators in the ring
+    int claim_ahead;    // the scheduler draws the next ticket when the weight loader has this many K-blocks left
     int w_group;        // weight K-blocks requested back to back
     int producer_ctas;  // CTAs with blockIdx.x < producer_ctas start at layer_begin, the rest one layer later
     int wait_flags;     // consumer prologue on/off
@@ -103,10 +129,13 @@ struct KernelParams {
 
 struct UnitInfo {
     int layer, m_blk, n_blk, ks, kb0, kb1, valid, tile;
-    int acquired, pad_[3];  // 1: the scheduler has already seen (and acquired) every ready counter of this unit
+    int acquired;  // 1: the scheduler has already seen (and acquired) every counter this unit depends on
+    int kind;      // kUnitMma | kUnitReduce (then kb0, kb1 = token columns)
+    int pad_[2];
 };
 
-__device__ __forceinline__ float act_apply(float x, int act) {
+template <int act>
+__device__ __forceinline__ float act_apply(float x) {
     if (act == kActRelu) return x > 0.0f ? x : 0.0f;
     if (act == kActGeluTanh) {
         float u = 0.7978845608028654f * (x + 0.044715f * x * x * x);
@@ -134,30 +163,158 @@ __device__ __forceinline__ void st_cg_f32(float* p, float v) {
     asm volatile("st.global.cg.f32 [%0], %1;" ::"l"(p), "f"(v) : "memory");
 }
 
-// Store 16 token columns (rows m_first .. m_first+15 of `out`) of this lane's output feature n as
-// bf16 (RNE).  Adjacent lanes hold adjacent n: lane pairs exchange one value per two columns so
-// that every lane stores a packed bf16x2 (even lanes the even column, odd lanes the odd one).
-__device__ __forceinline__ void store_out16(__nv_bfloat16* out, size_t ld, int n, bool n_ok, int m_first, int m_end,
-                                            const float (&f)[16]) {
-    const bool odd = (threadIdx.x & 1) != 0;
+__device__ __forceinline__ void st_cg_f32x4(float* p, float a, float b, float c, float d) {
+    asm volatile("st.global.cg.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+}
+__device__ __forceinline__ float4 ld_cg_f32x4(const float* p) {
+    float4 v;
+    asm volatile("ld.global.cg.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_shared_b16(uint32_t addr, uint16_t v) {
+    asm volatile("st.shared.b16 [%0], %1;" ::"r"(addr), "h"(v) : "memory");
+}
+__device__ __forceinline__ uint4 ld_shared_v4(uint32_t addr) {
+    uint4 v;
+    asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr) : "memory");
+    return v;
+}
+
+// Epilogue output path (steps a3 / a7).  The accumulator is feature-major (TMEM lane = output
+// feature n, column = token m) while the output is token-major, so a chunk of up to 32 token columns
+// of one 128-feature block is transposed through a shared-memory staging buffer: every thread
+// converts its feature's values (act, RNE to bf16) and writes them at stage[token][feature]; after a
+// barrier among the 128 epilogue threads the buffer leaves as 16-byte pieces, a warp storing two
+// complete 256-byte output rows per instruction.  Two buffers alternate (`parity`), so one barrier
+// per chunk suffices: a buffer is rewritten only after the barrier of the chunk in between.
+template <int kCols, int kAct>
+__device__ __forceinline__ void stage_cols(const uint32_t (&f)[kCols], uint32_t buf, int r) {
+    // the activation is a compile-time choice here: a run-time switch per element would serialise the
+    // 32 independent columns behind one another's MUFU latency
 #pragma unroll
-    for (int j = 0; j < 16; j += 2) {
-        const uint32_t a = __bfloat16_as_ushort(__float2bfloat16_rn(f[j]));
-        const uint32_t b = __bfloat16_as_ushort(__float2bfloat16_rn(f[j + 1]));
-        const uint32_t recv = __shfl_xor_sync(0xffffffffu, odd ? a : b, 1);
-        const int m = m_first + j + (odd ? 1 : 0);
-        const uint32_t packed = odd ? (recv | (b << 16)) : (a | (recv << 16));
-        if (n_ok && m < m_end)
-            *reinterpret_cast<uint32_t*>(out + static_cast<size_t>(m) * ld + (n & ~1)) = packed;
+    for (int j = 0; j < kCols; ++j)
+        st_shared_b16(buf + static_cast<uint32_t>(j * kTileN + r) * 2u, __bfloat16_as_ushort(__float2bfloat16_rn(act_apply<kAct>(__uint_as_float(f[j])))));
+}
+
+template <int kCols>
+__device__ __forceinline__ void emit_cols(const uint32_t (&f)[kCols], uint32_t stage_s, uint32_t& parity, int r,
+                                          __nv_bfloat16* out, size_t ld, int n_base, int N, int m_first, int m_end,
+                                          int act) {
+    const uint32_t buf = stage_s + (parity & 1u) * kStageBufBytes;
+    parity ^= 1u;
+    if (act == kActGeluTanh) stage_cols<kCols, kActGeluTanh>(f, buf, r);
+    else if (act == kActRelu) stage_cols<kCols, kActRelu>(f, buf, r);
+    else stage_cols<kCols, kActNone>(f, buf, r);
+    bar_sync(1, kEpiThreads);
+#pragma unroll
+    for (int p = 0; p < kCols * 16 / kEpiThreads; ++p) {
+        const int piece = p * kEpiThreads + r;  // 16 pieces of 8 features per token row
+        const int j = piece >> 4, q = piece & 15;
+        const int m = m_first + j, n = n_base + q * 8;
+        if (m < m_end && n < N) {
+            const uint4 v = ld_shared_v4(buf + static_cast<uint32_t>(j * kTileN + q * 8) * 2u);
+            *reinterpret_cast<uint4*>(out + static_cast<size_t>(m) * ld + n) = v;
+        }
     }
 }
 
-// Spin until *ctr has reached `target` (wrap-safe).  Relaxed polls + one acquire fence = acquire pattern.
-// Bounded: after timeout_ns (or when another waiter has already given up) the wait is abandoned, the
-// device status word records it, and `true` is returned so that the caller stops waiting for good.
-__device__ __forceinline__ bool poll_counter(const uint32_t* ctr, uint32_t target, uint32_t* status,
+// Sum 16 token columns [c, c+16) of feature r over the `split` partials of one 128-row block, always in
+// slice order 0..split-1 (the rounding never depends on who reduces, nor on arrival order).  `blk` points
+// at slice 0; slices are `ks_stride` floats apart; layout inside a slice block: [column / 4][128][4].
+__device__ __forceinline__ void gather16(const float* blk, int split, size_t ks_stride, int c, int r, float (&sum)[16]) {
+    const float* p0 = blk + (static_cast<size_t>(c >> 2) * kTileN + r) * 4;
+    for (int ks = 0; ks < split; ks += kGather) {
+        float4 t[kGather][4];
+#pragma unroll
+        for (int q = 0; q < kGather; ++q)
+            if (ks + q < split) {
+#pragma unroll
+                for (int g = 0; g < 4; ++g) t[q][g] = ld_cg_f32x4(p0 + (ks + q) * ks_stride + static_cast<size_t>(g) * kTileN * 4);
+            }
+#pragma unroll
+        for (int q = 0; q < kGather; ++q)
+            if (ks + q < split) {
+                if (ks + q == 0) {
+#pragma unroll
+                    for (int g = 0; g < 4; ++g) {
+                        sum[4 * g] = t[q][g].x; sum[4 * g + 1] = t[q][g].y; sum[4 * g + 2] = t[q][g].z; sum[4 * g + 3] = t[q][g].w;
+                    }
+                } else {
+#pragma unroll
+                    for (int g = 0; g < 4; ++g) {
+                        sum[4 * g] += t[q][g].x; sum[4 * g + 1] += t[q][g].y; sum[4 * g + 2] += t[q][g].z; sum[4 * g + 3] += t[q][g].w;
+                    }
+                }
+            }
+    }
+}
+
+template <int kC>
+__device__ __forceinline__ void tmem_ld_cols(uint32_t taddr, uint32_t (&v)[kC]);
+template <>
+__device__ __forceinline__ void tmem_ld_cols<16>(uint32_t taddr, uint32_t (&v)[16]) { tmem_ld16(taddr, v); }
+template <>
+__device__ __forceinline__ void tmem_ld_cols<32>(uint32_t taddr, uint32_t (&v)[32]) { tmem_ld32(taddr, v); }
+
+// Context of one epilogue thread's output path.
+struct EmitCtx {
+    uint32_t stage_s;
+    int r;
+    __nv_bfloat16* out;
+    size_t ld;
+    int n_first, N, m0, m_end, act, tile_m;
+};
+
+__device__ __forceinline__ void release_acc(uint32_t bar) {
+    tc_fence_before();
+    mbar_arrive(bar);
+}
+
+template <int kC>
+__device__ __forceinline__ void emit_chunk(const uint32_t (&v)[kC], int cc, const EmitCtx& e, uint32_t& parity) {
+    const int rr = cc >= e.tile_m ? 1 : 0, c = cc - rr * e.tile_m;
+    emit_cols<kC>(v, e.stage_s, parity, e.r, e.out, e.ld, e.n_first + rr * kTileN, e.N, e.m0 + c, e.m_end, e.act);
+}
+
+template <int kC>
+__device__ __forceinline__ void store_chunk(const uint32_t (&v)[kC], int cc, float* wsp) {
+#pragma unroll
+    for (int g = 0; g < kC / 4; ++g)
+        st_cg_f32x4(wsp + static_cast<size_t>((cc >> 2) + g) * kTileN * 4, __uint_as_float(v[4 * g]), __uint_as_float(v[4 * g + 1]),
+                    __uint_as_float(v[4 * g + 2]), __uint_as_float(v[4 * g + 3]));
+}
+
+// Drain one accumulator (`total` TMEM columns from taddr) in chunks of kC columns: the tcgen05.ld of the next
+// chunk is in flight while the current one is consumed -- kDirect: act + bf16 + transposed store of the output
+// (steps a3 / a7), else: fp32 split-K partial (step a8); once the last chunk has been read the accumulator is
+// handed back to the MMA warp (bar_release = tempty).
+template <int kC, bool kDirect>
+__device__ __forceinline__ void drain_acc(uint32_t taddr, int total, uint32_t bar_release, const EmitCtx& e, uint32_t& parity,
+                                          float* wsp) {
+    uint32_t va[kC], vb[kC];
+    tmem_ld_cols<kC>(taddr, va);
+    for (int cc = 0; cc < total; cc += 2 * kC) {
+        tmem_ld_wait();
+        const bool more = cc + kC < total;
+        if (more) tmem_ld_cols<kC>(taddr + cc + kC, vb);
+        else release_acc(bar_release);
+        if (kDirect) emit_chunk<kC>(va, cc, e, parity);
+        else store_chunk<kC>(va, cc, wsp);
+        if (more) {
+            tmem_ld_wait();
+            if (cc + 2 * kC < total) tmem_ld_cols<kC>(taddr + cc + 2 * kC, va);
+            else release_acc(bar_release);
+            if (kDirect) emit_chunk<kC>(vb, cc + kC, e, parity);
+            else store_chunk<kC>(vb, cc + kC, wsp);
+        }
+    }
+}
+
+// Spin until *ctr has reached `target` (wrap-safe), then acquire.  Relaxed polls + one acquire fence =
+// acquire pattern.  Bounded: after timeout_ns (or when another waiter has already given up) the wait is
+// abandoned, the device status word records it and the caller carries on (output undefined, kernel ends).
+__device__ __forceinline__ void poll_counter(const uint32_t* ctr, uint32_t target, uint32_t* status,
                                              unsigned long long timeout_ns, unsigned long long& waited) {
-    bool gave_up = false;
     if (static_cast<int32_t>(ld_relaxed_gpu(ctr) - target) < 0) {
         const long long c0 = clock64();
         const uint64_t t0 = globaltimer_ns();
@@ -165,10 +322,9 @@ __device__ __forceinline__ bool poll_counter(const uint32_t* ctr, uint32_t targe
         while (static_cast<int32_t>(ld_relaxed_gpu(ctr) - target) < 0) {
             __nanosleep(32);
             if ((++n & 255u) == 0) {
-                if (ld_relaxed_gpu(status) != 0) { gave_up = true; break; }
+                if (ld_relaxed_gpu(status) != 0) break;
                 if (globaltimer_ns() - t0 > timeout_ns) {
                     atomicCAS(status, 0u, kStatusFlagTimeout);
-                    gave_up = true;
                     break;
                 }
             }
@@ -176,7 +332,6 @@ __device__ __forceinline__ bool poll_counter(const uint32_t* ctr, uint32_t targe
         waited += static_cast<unsigned long long>(clock64() - c0);
     }
     fence_acq_rel_gpu();
-    return gave_up;
 }
 
 __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_constant__ KernelParams P) {
@@ -185,14 +340,18 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
     uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
 
     const int tile_m = P.tile_m;
+    const int n_sub = P.n_sub;
+    const int tile_n = kTileN * n_sub;  // weight rows per unit
+    const uint32_t w_tile_bytes = static_cast<uint32_t>(n_sub) * kWTileBytes;
     const uint32_t a_tile_bytes = static_cast<uint32_t>(tile_m) * (kTileK * 2);
     const int stages = P.stages;      // weight ring depth
     const int a_stages = P.a_stages;  // activation ring depth (its own, deeper ring: the consumer prologue's
                                       // polls and fences then run K-blocks ahead of the weight stream)
-    const uint32_t a_ring = smem_base + static_cast<uint32_t>(stages) * kWTileBytes;
-    const uint32_t ring_bytes = static_cast<uint32_t>(stages) * kWTileBytes + static_cast<uint32_t>(a_stages) * a_tile_bytes;
+    const uint32_t a_ring = smem_base + static_cast<uint32_t>(stages) * w_tile_bytes;
+    const uint32_t stage_s = a_ring + static_cast<uint32_t>(a_stages) * a_tile_bytes;  // epilogue staging
+    const uint32_t ring_bytes = static_cast<uint32_t>(stages) * w_tile_bytes + static_cast<uint32_t>(a_stages) * a_tile_bytes + kStageBytes;
 
-    // control block after the two rings
+    // control block after the rings
     uint8_t* ctrl = smem_gen + ring_bytes;
     const uint32_t ctrl_s = smem_base + ring_bytes;
     const uint32_t bar_full = ctrl_s;                          // [kMaxStages]  weight tile landed
@@ -209,6 +368,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
     volatile uint32_t* s_tmem = reinterpret_cast<volatile uint32_t*>(ctrl + kBarBytes + sizeof(UnitInfo) * kSchedSlots);
     volatile uint32_t* s_last = s_tmem + 1;
     volatile unsigned long long* s_epoch = reinterpret_cast<volatile unsigned long long*>(s_tmem + 2);
+    volatile uint32_t* s_pre = s_tmem + 4;  // [0] weight / [1] activation K-blocks of the first unit requested during setup
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
@@ -216,11 +376,12 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
     CtaStats* const my_stats = P.stats + blockIdx.x;
     if (threadIdx.x == 0) my_stats->ts[0] = globaltimer_ns();
 
-    // TMEM accumulator ring: as many tile_m-column accumulators as fit (<= 8), so that the MMA warp can
-    // run ahead of an epilogue that is waiting on a memory round trip
+    // TMEM accumulator ring: as many (n_sub x tile_m)-column accumulators as fit (<= 8), so that the MMA
+    // warp can run ahead of an epilogue that is waiting on a memory round trip
     const uint32_t acc_stages = static_cast<uint32_t>(P.acc_stages);
+    const uint32_t acc_cols = static_cast<uint32_t>(n_sub * tile_m);
     uint32_t tmem_cols = 32;
-    while (tmem_cols < acc_stages * static_cast<uint32_t>(tile_m)) tmem_cols <<= 1;
+    while (tmem_cols < acc_stages * acc_cols) tmem_cols <<= 1;
 
     // ------------------------------------------------------------------ one-time setup
     if (threadIdx.x == 0) {
@@ -232,6 +393,19 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
         }
     }
     if (threadIdx.x == 32) {
+        // This thread is the weight loader.  The first unit of the CTA is static (same rule as in the
+        // scheduler below), so its first ring of weight tiles -- and, if it has no producers, of activation
+        // tiles -- is requested right here, before TMEM allocation and the CTA-wide sync: the first bytes are
+        // in flight ~1 us earlier.
+        int l0 = P.layer_begin;
+        uint32_t sid = blockIdx.x;
+        if (static_cast<int>(blockIdx.x) >= P.producer_ctas && P.layer_begin + 1 < P.layer_end) {
+            l0 = P.layer_begin + 1;
+            sid = blockIdx.x - P.producer_ctas;
+        }
+        const bool have = sid < static_cast<uint32_t>(P.layer[l0].units);
+        uint2 raw = make_uint2(0u, 0u);
+        if (have) raw = __ldg(reinterpret_cast<const uint2*>(P.layer[l0].table) + sid);  // in flight during the inits
         for (int s = 0; s < stages; ++s) {
             mbar_init(bar_full + 8 * s, 1);
             mbar_init(bar_empty + 8 * s, 1);
@@ -250,6 +424,30 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
             mbar_init(bar_wtaken + 8 * i, 1);
         }
         fence_mbar_init();
+        uint32_t pre_w = 0, pre_a = 0;
+        if (have && ((raw.x >> 16) & 0xffu) == kUnitMma && !(P.flags & 0x100u)) {
+            fence_proxy_async();  // the barrier inits (generic proxy) before the TMA unit's complete_tx on them
+            const int tile = static_cast<int>(raw.x & 0xffffu), kb0 = static_cast<int>(raw.y & 0xffffu), kb1 = static_cast<int>(raw.y >> 16);
+            const int n_blk = tile % P.layer[l0].n_blks, m_blk = tile / P.layer[l0].n_blks;
+            const uint64_t pol = policy_evict_first();
+            pre_w = static_cast<uint32_t>(min(stages, kb1 - kb0));
+            my_stats->ts[3] = globaltimer_ns();
+            for (uint32_t i = 0; i < pre_w; ++i) {
+                mbar_arrive_expect_tx(bar_full + 8 * i, w_tile_bytes);
+                if (!(P.flags & kFlagNoEvictFirst))
+                    tma_load_2d_hint(smem_base + i * w_tile_bytes, &P.tm_w[l0], (kb0 + static_cast<int>(i)) * kTileK, n_blk * tile_n, bar_full + 8 * i, pol);
+                else tma_load_2d(smem_base + i * w_tile_bytes, &P.tm_w[l0], (kb0 + static_cast<int>(i)) * kTileK, n_blk * tile_n, bar_full + 8 * i);
+            }
+            if (l0 == P.layer_begin) {  // input of the launch: nothing to wait for
+                pre_a = static_cast<uint32_t>(min(a_stages, kb1 - kb0));
+                for (uint32_t i = 0; i < pre_a; ++i) {
+                    mbar_arrive_expect_tx(bar_afull + 8 * i, a_tile_bytes);
+                    tma_load_2d(a_ring + i * a_tile_bytes, &P.tm_a[l0], (kb0 + static_cast<int>(i)) * kTileK, P.m_off + m_blk * tile_m, bar_afull + 8 * i);
+                }
+            }
+        }
+        s_pre[0] = pre_w;
+        s_pre[1] = pre_a;
     }
     if (warp == 3) {
         tmem_alloc(smem_u32(const_cast<uint32_t*>(s_tmem)), tmem_cols);
@@ -282,7 +480,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
             while (!finished) {
                 UnitInfo u;
                 u.valid = 0;
-                u.layer = u.m_blk = u.n_blk = u.ks = u.kb0 = u.kb1 = u.tile = u.acquired = 0;
+                u.layer = u.m_blk = u.n_blk = u.ks = u.kb0 = u.kb1 = u.tile = u.acquired = u.kind = 0;
                 // claim at most one unit ahead of the W loader (keeps the tail balanced)
                 if (it >= 1) mbar_wait(bar_wtaken + 8 * ((it - 1) % kSchedSlots), ((it - 1) / kSchedSlots) & 1);
                 while (l < P.layer_end) {
@@ -299,33 +497,33 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                         ++l;
                         continue;
                     }
-                    if ((P.flags & kFlagDebugReverse) && l == P.layer_begin) t = L.units - 1 - t;
-                    const int tiles = L.n_blks * P.m_blks;
-                    int tile, ks;
-                    if (!L.ks_major) {
-                        tile = t / L.split;
-                        ks = t % L.split;
-                    } else {  // K-slice-major: early units depend on early producer tiles only
-                        ks = t / tiles;
-                        tile = t % tiles;
-                    }
+                    const uint2 raw = __ldg(reinterpret_cast<const uint2*>(L.table) + t);
                     u.layer = l;
-                    u.tile = tile;
-                    u.m_blk = tile / L.n_blks;
-                    u.n_blk = tile % L.n_blks;
-                    u.ks = ks;
-                    u.kb0 = __ldg(L.kb_bounds + ks);
-                    u.kb1 = __ldg(L.kb_bounds + ks + 1);
+                    u.tile = static_cast<int>(raw.x & 0xffffu);
+                    u.kind = static_cast<int>((raw.x >> 16) & 0xffu);
+                    u.ks = static_cast<int>(raw.x >> 24);
+                    u.kb0 = static_cast<int>(raw.y & 0xffffu);
+                    u.kb1 = static_cast<int>(raw.y >> 16);
+                    u.m_blk = u.tile / L.n_blks;
+                    u.n_blk = u.tile % L.n_blks;
                     u.valid = 1;
-                    if (P.wait_flags && l > P.layer_begin && !(P.flags & 0x80u)) {
+                    if (u.kind == kUnitReduce) {
+                        // fast path of a reduce unit: all slices of its tile have already arrived
+                        const uint32_t target = static_cast<uint32_t>((epoch + 1ull) * static_cast<unsigned long long>(L.split));
+                        if (static_cast<int32_t>(ld_relaxed_gpu(L.arrive + u.tile) - target) >= 0) {
+                            fence_acq_rel_gpu();
+                            u.acquired = 1;
+                        }
+                    } else if (P.wait_flags && l > P.layer_begin && !(P.flags & 0x80u)) {
                         // Consumer prologue, fast path (the prologue lives in the scheduler
                         // warp): one look at all ready counters under this unit's K range.  If every producer
                         // tile is already published -- the normal case, the scheduler runs a unit ahead --
                         // ONE acquire fence here covers the whole unit and the loaders never poll.  Otherwise
                         // the activation loader polls slice by slice while the weight loader prefetches.
-                        const uint32_t target = static_cast<uint32_t>(epoch + 1ull);
-                        const uint32_t* rd = P.layer[l - 1].ready + u.m_blk * P.layer[l - 1].n_blks;
-                        const int s0 = (u.kb0 * kTileK) / kTileN, s1 = ((u.kb1 - 1) * kTileK) / kTileN + 1;
+                        const LayerParams& Lp = P.layer[l - 1];
+                        const uint32_t target = static_cast<uint32_t>((epoch + 1ull) * static_cast<unsigned long long>(Lp.ready_inc));
+                        const uint32_t* rd = Lp.ready + u.m_blk * Lp.n_blks;
+                        const int s0 = (u.kb0 * kTileK) / tile_n, s1 = ((u.kb1 - 1) * kTileK) / tile_n + 1;
                         bool all = (s1 - s0) <= 32;
                         for (int sb = s0; sb < s1 && all; sb += 8) {
                             uint32_t v[8];
@@ -363,31 +561,51 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 const uint32_t slot = it % kSchedSlots;
                 mbar_wait(bar_sfull + 8 * slot, (it / kSchedSlots) & 1);
                 const UnitInfo u = ring[slot];
-                mbar_arrive(bar_wtaken + 8 * slot);
                 mbar_arrive(bar_sempty + 8 * slot);
+                // Late binding: the scheduler may draw the NEXT ticket only once this unit has at most
+                // claim_ahead K-blocks left to request.  A unit stalled on its producers (the ring is full, the
+                // MMA warp waits for the activation loader) therefore never holds a second ticket.
+                // (For a reduce unit the epilogue warps give the go once its partials have arrived.)
+                bool told = u.kind == kUnitReduce || !u.valid || u.kb1 - u.kb0 <= P.claim_ahead;
+                if (told && u.kind != kUnitReduce) mbar_arrive(bar_wtaken + 8 * slot);
                 if (!u.valid) break;
                 if (it < kUnitTrace) {
                     my_stats->unit_ts[it][0] = globaltimer_ns();
-                    my_stats->unit_id[it] = (static_cast<uint32_t>(u.layer) << 28) | (static_cast<uint32_t>(u.tile) << 8) | static_cast<uint32_t>(u.ks);
+                    my_stats->unit_id[it] = (static_cast<uint32_t>(u.layer) << 28) | (static_cast<uint32_t>(u.tile) << 8) |
+                                            static_cast<uint32_t>(u.kind == kUnitReduce ? 0x80 | (u.kb0 >> 4) : u.ks);
+                }
+                if (u.kind == kUnitReduce) {
+                    if (it < kUnitTrace) my_stats->unit_ts[it][1] = my_stats->unit_ts[it][0];
+                    continue;
                 }
                 const CUtensorMap* tm = &P.tm_w[u.layer];
                 // K-blocks are requested in groups of w_group: the loader first waits until the whole group of
                 // stages is free and then issues the group back to back, so that the 128-byte pieces of one
                 // weight row that are adjacent in memory reach the DRAM controller together
-                for (int kb = u.kb0; kb < u.kb1;) {
+                int kb = u.kb0;
+                if (it == 0) {  // the first ring of this unit was requested during setup
+                    const uint32_t pre = s_pre[0];
+                    kb += static_cast<int>(pre);
+                    stage = pre % static_cast<uint32_t>(stages);
+                    phase = pre / static_cast<uint32_t>(stages);
+                }
+                while (kb < u.kb1) {
                     const int g = min(P.w_group, u.kb1 - kb);
                     uint32_t st = stage, ph = phase;
                     for (int i = 0; i < g; ++i) {
                         mbar_wait_timed(bar_empty + 8 * st, ph ^ 1, w_wait);
                         if (++st == static_cast<uint32_t>(stages)) { st = 0; ph ^= 1; }
                     }
+                    if (!told && u.kb1 - kb <= P.claim_ahead) {
+                        told = true;
+                        mbar_arrive(bar_wtaken + 8 * slot);
+                    }
                     for (int i = 0; i < g; ++i, ++kb) {
                         const uint32_t full = bar_full + 8 * stage;
-                        mbar_arrive_expect_tx(full, kWTileBytes);
-                        const uint32_t dst = smem_base + stage * kWTileBytes;
-                        if (hint) tma_load_2d_hint(dst, tm, kb * kTileK, u.n_blk * kTileN, full, pol);
-                        else tma_load_2d(dst, tm, kb * kTileK, u.n_blk * kTileN, full);
-                        if (it == 0 && kb == u.kb0) my_stats->ts[3] = globaltimer_ns();
+                        mbar_arrive_expect_tx(full, w_tile_bytes);
+                        const uint32_t dst = smem_base + stage * w_tile_bytes;
+                        if (hint) tma_load_2d_hint(dst, tm, kb * kTileK, u.n_blk * tile_n, full, pol);
+                        else tma_load_2d(dst, tm, kb * kTileK, u.n_blk * tile_n, full);
                         if (++stage == static_cast<uint32_t>(stages)) { stage = 0; phase ^= 1; }
                     }
                 }
@@ -401,30 +619,39 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
             uint32_t stage = 0, phase = 0;
             unsigned long long stall = 0, polls = 0;
             bool aborted = false;
-            const uint32_t target = static_cast<uint32_t>(epoch + 1ull);
             for (uint32_t it = 0;; ++it) {
                 const uint32_t slot = it % kSchedSlots;
                 mbar_wait(bar_sfull + 8 * slot, (it / kSchedSlots) & 1);
                 const UnitInfo u = ring[slot];
                 mbar_arrive(bar_sempty + 8 * slot);
                 if (!u.valid) break;
+                if (u.kind == kUnitReduce) continue;
                 const CUtensorMap* tm = &P.tm_a[u.layer];
                 const bool wait = P.wait_flags && u.layer > P.layer_begin && !u.acquired;
                 if (P.wait_flags && u.layer > P.layer_begin) fence_proxy_async();
-                const uint32_t* ready = wait ? P.layer[u.layer - 1].ready + u.m_blk * P.layer[u.layer - 1].n_blks : nullptr;
+                const LayerParams& Lp = P.layer[u.layer > 0 ? u.layer - 1 : 0];
+                const uint32_t target = static_cast<uint32_t>((epoch + 1ull) * static_cast<unsigned long long>(Lp.ready_inc));
+                const uint32_t* ready = wait ? Lp.ready + u.m_blk * Lp.n_blks : nullptr;
                 // Slices [.., ready_upto) of this unit are known to be published.  Readiness is monotone
                 // within a run, so the prologue looks ahead: up to 8 counters are read with independent
                 // relaxed loads that are ISSUED a few K-blocks before their result is needed (the round trip
                 // overlaps the TMA issue of slices already known to be ready), then one acquire fence turns
                 // the observations into an acquire pattern (PTX memory model: relaxed read + fence.acq_rel).
-                const int slice_end = wait ? ((u.kb1 - 1) * kTileK) / kTileN + 1 : 0;
-                int ready_upto = wait ? (u.kb0 * kTileK) / kTileN : 0;
+                const int slice_end = wait ? ((u.kb1 - 1) * kTileK) / tile_n + 1 : 0;
+                int ready_upto = wait ? (u.kb0 * kTileK) / tile_n : 0;
                 uint32_t v[8];
                 int pend_base = -1;  // >= 0: v[] holds in-flight reads of counters pend_base .. pend_base+7
-                for (int kb = u.kb0; kb < u.kb1; ++kb) {
+                int kb_first = u.kb0;
+                if (it == 0) {
+                    const uint32_t pre = s_pre[1];
+                    kb_first += static_cast<int>(pre);
+                    stage = pre % static_cast<uint32_t>(a_stages);
+                    phase = pre / static_cast<uint32_t>(a_stages);
+                }
+                for (int kb = kb_first; kb < u.kb1; ++kb) {
                     mbar_wait(bar_aempty + 8 * stage, phase ^ 1);
                     if (wait) {
-                        const int slice = (kb * kTileK) / kTileN;  // producer tile that wrote these columns
+                        const int slice = (kb * kTileK) / tile_n;  // producer tile that wrote these columns
                         if (pend_base < 0 && ready_upto < slice_end && slice + 2 >= ready_upto) {
                             pend_base = ready_upto;
 #pragma unroll
@@ -480,30 +707,37 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
             const uint32_t idesc = make_idesc_bf16(kTileN, tile_m);
             uint32_t stage = 0, phase = 0, astage = 0, aphase = 0;
             unsigned long long wait_ops = 0, wait_acc = 0;
+            uint32_t mma_it = 0;  // MMA units so far: picks the accumulator (the epilogue warps count alike)
             for (uint32_t it = 0;; ++it) {
                 const uint32_t slot = it % kSchedSlots;
                 mbar_wait(bar_sfull + 8 * slot, (it / kSchedSlots) & 1);
                 const UnitInfo u = ring[slot];
                 mbar_arrive(bar_sempty + 8 * slot);
                 if (!u.valid) break;
-                const uint32_t acc = it % acc_stages;
-                mbar_wait_timed(bar_tempty + 8 * acc, ((it / acc_stages) & 1u) ^ 1u, wait_acc);
+                if (u.kind == kUnitReduce) continue;
+                const uint32_t acc = mma_it % acc_stages;
+                mbar_wait_timed(bar_tempty + 8 * acc, ((mma_it / acc_stages) & 1u) ^ 1u, wait_acc);
+                ++mma_it;
                 tc_fence_after();
-                const uint32_t d_tmem = tmem_base + acc * static_cast<uint32_t>(tile_m);
+                const uint32_t d_tmem = tmem_base + acc * acc_cols;
                 for (int kb = u.kb0; kb < u.kb1; ++kb) {
                     mbar_wait_timed(bar_afull + 8 * astage, aphase, wait_ops);
                     mbar_wait_timed(bar_full + 8 * stage, phase, wait_ops);
                     tc_fence_after();
                     if (it == 0 && kb == u.kb0) my_stats->ts[4] = globaltimer_ns();
-                    const uint32_t a_addr = smem_base + stage * kWTileBytes;
+                    const uint32_t a_addr = smem_base + stage * w_tile_bytes;
                     const uint32_t b_addr = a_ring + astage * a_tile_bytes;
-                    const uint64_t a_desc = make_smem_desc_sw128(a_addr);
                     const uint64_t b_desc = make_smem_desc_sw128(b_addr);
+                    for (int rr = 0; rr < n_sub; ++rr) {
+                        // block rr = weight rows [128 rr, 128 rr + 128) of the stage, accumulator columns
+                        // [rr tile_m, (rr + 1) tile_m); both blocks read the same activation tile
+                        const uint64_t a_desc = make_smem_desc_sw128(a_addr + rr * kWTileBytes);
 #pragma unroll
-                    for (int k = 0; k < kTileK / kUmmaK; ++k) {
-                        // advancing K by 16 bf16 = 32 B inside the 128 B swizzle span: +2 in the
-                        // (addr >> 4) field of the descriptor
-                        umma_bf16(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb > u.kb0 || k > 0) ? 1u : 0u);
+                        for (int k = 0; k < kTileK / kUmmaK; ++k) {
+                            // advancing K by 16 bf16 = 32 B inside the 128 B swizzle span: +2 in the
+                            // (addr >> 4) field of the descriptor
+                            umma_bf16(d_tmem + rr * tile_m, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb > u.kb0 || k > 0) ? 1u : 0u);
+                        }
                     }
                     umma_commit(bar_empty + 8 * stage);
                     umma_commit(bar_aempty + 8 * astage);
@@ -517,9 +751,10 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
         }
     } else {
         // ===== epilogue warps 4..7 (steps a3, a4, a7, a8)
-        const int r = threadIdx.x - (kThreads - kEpiThreads);  // TMEM lane = weight row inside the tile
+        const int r = threadIdx.x - (kThreads - kEpiThreads);  // TMEM lane = weight row inside a 128-row block
         const int wq = r >> 5;
-        unsigned long long wait_acc = 0, wait_part = 0;
+        unsigned long long wait_acc = 0, wait_part = 0, t_gather = 0, t_partial = 0, t_direct = 0;
+        uint32_t mma_it = 0, parity = 0;
         for (uint32_t it = 0;; ++it) {
             const uint32_t slot = it % kSchedSlots;
             mbar_wait(bar_sfull + 8 * slot, (it / kSchedSlots) & 1);
@@ -527,95 +762,87 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
             mbar_arrive(bar_sempty + 8 * slot);
             if (!u.valid) break;
             const LayerParams& L = P.layer[u.layer];
-            const uint32_t acc = it % acc_stages;
-            const uint32_t taddr = tmem_base + (static_cast<uint32_t>(wq * 32) << 16) + acc * static_cast<uint32_t>(tile_m);
-            const int n = u.n_blk * kTileN + r;
             const int m0 = P.m_off + u.m_blk * tile_m;
-            const bool n_ok = n < L.N;
             const size_t out_row = static_cast<size_t>(L.N);
-            const size_t ks_stride = static_cast<size_t>(tile_m) * kTileN;
-            float* const ws_tile = L.ws + static_cast<size_t>(u.tile) * L.split * ks_stride + r;
-            mbar_wait_timed(bar_tfull + 8 * acc, (it / acc_stages) & 1u, wait_acc);
-            tc_fence_after();
-            if (it == 0 && r == 0) my_stats->ts[5] = globaltimer_ns();
-            if (it < kUnitTrace && r == 0) my_stats->unit_ts[it][2] = globaltimer_ns();
-            if (L.split == 1) {
-                for (int c0 = 0; c0 < tile_m; c0 += 16) {
-                    uint32_t v[16];
-                    tmem_ld16(taddr + c0, v);
-                    tmem_ld_wait();
-                    if (c0 + 16 >= tile_m) {  // accumulator fully read: hand TMEM back to the MMA warp
-                        tc_fence_before();
-                        mbar_arrive(bar_tempty + 8 * acc);
-                    }
-                    float sum[16];
-#pragma unroll
-                    for (int j = 0; j < 16; ++j) sum[j] = act_apply(__uint_as_float(v[j]), L.act);
-                    store_out16(L.out, out_row, n, n_ok, m0 + c0, P.m_end, sum);
+            const size_t blk_stride = static_cast<size_t>(tile_m) * kTileN;        // floats per 128-row block of a partial
+            const size_t ks_stride = blk_stride * n_sub;                           // floats per slice
+            float* const ws_tile = L.ws + static_cast<size_t>(u.tile) * L.split * ks_stride;
+            bool stored = false;  // this unit wrote (part of) the layer's output
+            int red_c0 = 0, red_c1 = 0;  // token columns of the tile whose partials this unit sums (none if equal)
+            if (u.kind == kUnitReduce) {
+                // ---- step a8, distributed form: sum the partials of token columns [kb0, kb1) of the tile
+                if (it < kUnitTrace && r == 0) my_stats->unit_ts[it][2] = globaltimer_ns();
+                if (!u.acquired) {
+                    if (r == 0)
+                        poll_counter(L.arrive + u.tile, static_cast<uint32_t>((epoch + 1ull) * static_cast<unsigned long long>(L.split)),
+                                     P.status, P.timeout_ns, wait_part);
+                    bar_sync(1, kEpiThreads);  // thread 0's acquire happens-before everybody's loads below
                 }
+                if (r == 0) mbar_arrive(bar_wtaken + 8 * slot);  // late binding: now the scheduler may draw the next ticket
+                red_c0 = u.kb0;
+                red_c1 = u.kb1;
             } else {
-                // ---- step a8 (split-K): every slice stores its fp32 partial and arrives on the tile's counter;
-                // whoever arrives LAST sums all partials in fixed slice order (so the rounding does not depend
-                // on who that is) and finishes the tile.  Nobody ever waits, so a slow slice delays only its
-                // own tile, never the epilogue warps of another CTA.
-                float* wsp = ws_tile + static_cast<size_t>(u.ks) * ks_stride;
-                for (int c0 = 0; c0 < tile_m; c0 += 16) {
-                    uint32_t v[16];
-                    tmem_ld16(taddr + c0, v);
-                    tmem_ld_wait();
-                    if (c0 + 16 >= tile_m) {
-                        tc_fence_before();
-                        mbar_arrive(bar_tempty + 8 * acc);
+                const uint32_t acc = mma_it % acc_stages;
+                const uint32_t taddr = tmem_base + (static_cast<uint32_t>(wq * 32) << 16) + acc * acc_cols;
+                mbar_wait_timed(bar_tfull + 8 * acc, (mma_it / acc_stages) & 1u, wait_acc);
+                ++mma_it;
+                tc_fence_after();
+                if (it == 0 && r == 0) my_stats->ts[5] = globaltimer_ns();
+                if (it < kUnitTrace && r == 0) my_stats->unit_ts[it][2] = globaltimer_ns();
+                const long long te0 = clock64();
+                if (L.split == 1) {
+                    const EmitCtx e{stage_s, r, L.out, out_row, u.n_blk * tile_n, L.N, m0, P.m_end, L.act, tile_m};
+                    drain_acc<16, true>(taddr, static_cast<int>(acc_cols), bar_tempty + 8 * acc, e, parity, nullptr);
+                    stored = true;
+                    t_direct += static_cast<unsigned long long>(clock64() - te0);
+                } else {
+                    // ---- step a8 (split-K): every slice stores its fp32 partial (16-byte pieces, a warp
+                    // writes 512 contiguous bytes) and arrives on the tile's counter.
+                    // (the columns of the n_sub blocks are consecutive both in TMEM and in the partial)
+                    float* wsp = ws_tile + static_cast<size_t>(u.ks) * ks_stride + static_cast<size_t>(r) * 4;
+                    const EmitCtx e{};
+                    drain_acc<16, false>(taddr, static_cast<int>(acc_cols), bar_tempty + 8 * acc, e, parity, wsp);
+                    // the 128 threads' partial stores happen-before thread 0's atomic (bar.sync); its release half
+                    // is cumulative and publishes the CTA's whole partial, its acquire half (on the last arrival)
+                    // makes the other slices' partials visible to the loads after the second barrier
+                    bar_sync(1, kEpiThreads);
+                    t_partial += static_cast<unsigned long long>(clock64() - te0);
+                    if (L.reduce_mode == kReduceLastArriver) {
+                        // whoever arrives LAST sums all partials in fixed slice order and finishes the tile.
+                        // Nobody ever waits, so a slow slice delays only its own tile.
+                        if (r == 0) {
+                            const uint32_t base = static_cast<uint32_t>(epoch * static_cast<unsigned long long>(L.split));
+                            const uint32_t old = atom_add_acq_rel_gpu(L.arrive + u.tile, 1u) - base;
+                            *s_last = (old == static_cast<uint32_t>(L.split - 1)) ? 1u : 0u;
+                        }
+                        bar_sync(1, kEpiThreads);
+                        const bool last = (*s_last != 0);
+                        bar_sync(1, kEpiThreads);  // s_last may be rewritten by the next unit only after all have read it
+                        if (last) red_c1 = tile_m;
+                    } else {
+                        // reduce units (their own tickets, later in this layer's table) finish the tile
+                        if (r == 0) red_release_gpu_add(L.arrive + u.tile, 1u);
                     }
-#pragma unroll
-                    for (int j = 0; j < 16; ++j) st_cg_f32(wsp + static_cast<size_t>(c0 + j) * kTileN, __uint_as_float(v[j]));
-                }
-                // the 128 threads' partial stores happen-before thread 0's atomic (bar.sync); its release half
-                // is cumulative and publishes the CTA's whole partial, its acquire half (on the last arrival)
-                // makes the other slices' partials visible to the loads after the second barrier
-                bar_sync(1, kEpiThreads);
-                if (r == 0) {
-                    const uint32_t base = static_cast<uint32_t>(epoch * static_cast<unsigned long long>(L.split));
-                    const uint32_t old = atom_add_acq_rel_gpu(L.arrive + u.tile, 1u) - base;
-                    *s_last = (old == static_cast<uint32_t>(L.split - 1)) ? 1u : 0u;
-                }
-                bar_sync(1, kEpiThreads);
-                const bool last = (*s_last != 0);
-                bar_sync(1, kEpiThreads);  // s_last may be rewritten by the next unit only after all have read it
-                if (!last) {
-                    if (it < kUnitTrace && r == 0) my_stats->unit_ts[it][3] = globaltimer_ns();
-                    continue;
-                }
-                for (int c0 = 0; c0 < tile_m; c0 += 16) {
-                    float sum[16];
-                    // up to 16 * kGather independent loads in flight per thread; the adds stay in slice order
-                    for (int ks = 0; ks < L.split; ks += kGather) {
-                        float t[kGather][16];
-#pragma unroll
-                        for (int q = 0; q < kGather; ++q)
-                            if (ks + q < L.split) {
-#pragma unroll
-                                for (int j = 0; j < 16; ++j)
-                                    t[q][j] = ld_cg_f32(ws_tile + (ks + q) * ks_stride + static_cast<size_t>(c0 + j) * kTileN);
-                            }
-#pragma unroll
-                        for (int q = 0; q < kGather; ++q)
-                            if (ks + q < L.split) {
-                                if (ks + q == 0) {
-#pragma unroll
-                                    for (int j = 0; j < 16; ++j) sum[j] = t[q][j];
-                                } else {
-#pragma unroll
-                                    for (int j = 0; j < 16; ++j) sum[j] += t[q][j];
-                                }
-                            }
-                    }
-#pragma unroll
-                    for (int j = 0; j < 16; ++j) sum[j] = act_apply(sum[j], L.act);
-                    store_out16(L.out, out_row, n, n_ok, m0 + c0, P.m_end, sum);
                 }
             }
-            if (L.publish) {
+            if (red_c1 > red_c0) {
+                const long long tg0 = clock64();
+                for (int rr = 0; rr < n_sub; ++rr) {
+                    const float* blk = ws_tile + rr * blk_stride;
+                    const int n_base = u.n_blk * tile_n + rr * kTileN;
+                    for (int c = red_c0; c < red_c1; c += 16) {
+                        float f[16];
+                        uint32_t w[16];
+                        gather16(blk, L.split, ks_stride, c, r, f);
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) w[j] = __float_as_uint(f[j]);
+                        emit_cols<16>(w, stage_s, parity, r, L.out, out_row, n_base, L.N, m0 + c, P.m_end, L.act);
+                    }
+                }
+                t_gather += static_cast<unsigned long long>(clock64() - tg0);
+                stored = true;
+            }
+            if (stored && L.publish) {
                 // producer epilogue (step a4; output tile, then fence, then the dependency
                 // update).  All four epilogue warps wrote the tile: their stores happen-before the
                 // barrier, and thread 0's gpu-scope release after it is cumulative (the pattern of a
@@ -635,6 +862,9 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
         if (r == 0) {
             my_stats->wait[4] = wait_acc;
             my_stats->wait[5] = wait_part;
+            my_stats->wait[1] = t_gather;
+            my_stats->wait[6] = t_partial;
+            my_stats->wait[7] = t_direct;
         }
     }
 

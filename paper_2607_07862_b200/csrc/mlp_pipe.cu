@@ -7,6 +7,7 @@
 #include <algorithm>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -42,12 +43,14 @@ struct mlp_pipe {
     int dev = 0, num_sms = 0;
     // resolved configuration
     int rows_per_launch = 0;  // M, or M / chunks
-    int tile_m = 0, m_blks = 0, stages = 0, a_stages = 0, grid = 0, producer_ctas = 0;
+    int tile_m = 0, m_blks = 0, n_sub = 1, stages = 0, a_stages = 0, acc_stages = 0, grid = 0, producer_ctas = 0;
     size_t smem_bytes = 0;
     int split[kMaxLayers] = {0};
-    int ks_major[kMaxLayers] = {0};
+    int reduce_mode[kMaxLayers] = {0};
+    int ready_inc[kMaxLayers] = {0};
     std::vector<int> bounds[kMaxLayers];       // K-block boundaries of the slices, split[l] + 1 entries
-    uint16_t* d_bounds[kMaxLayers] = {nullptr};  // the same on the device
+    std::vector<UnitDesc> table[kMaxLayers];   // ticket -> unit
+    UnitDesc* d_table[kMaxLayers] = {nullptr};  // the same on the device
     int tiles[kMaxLayers] = {0};
     // device memory owned by the handle
     __nv_bfloat16* H[kMaxLayers] = {nullptr};  // H[l] = output of layer l, l < L-1
@@ -139,71 +142,49 @@ int validate_mode(const mlp_mode& m, int M) {
     if (m.stages < 0 || m.split_k < 0 || m.grid < 0 || m.timeout_ms < 0 || m.w_group < 0) return MLP_ERR_INVALID;
     for (int l = 0; l < kMaxLayers; ++l)
         if (m.split_k_layer[l] < 0) return MLP_ERR_INVALID;
-    if (m.tile_m > 256 || (m.tile_n != 0 && m.tile_n != kTileN) || (m.tile_k != 0 && m.tile_k != kTileK) ||
+    if (m.tile_m > 256 || (m.tile_n != 0 && m.tile_n != kTileN && m.tile_n != 2 * kTileN) ||
+        (m.tile_n == 2 * kTileN && m.tile_m > 256) || (m.tile_k != 0 && m.tile_k != kTileK) ||
         (m.kslice_tiles != 0 && m.kslice_tiles != 1))
         return MLP_ERR_UNSUPPORTED;
     return MLP_OK;
 }
 
-// The launch configuration.
-void resolve(mlp_pipe* h) {
-    const mlp_mode& m = h->mode;
-    h->rows_per_launch = m.kind == MLP_MICROBATCH ? h->M / m.chunks : h->M;
-    if (m.tile_m > 0) {
-        h->tile_m = m.tile_m;
-        h->m_blks = ceil_div(h->rows_per_launch, h->tile_m);
-    } else {
-        h->m_blks = ceil_div(h->rows_per_launch, 256);
-        h->tile_m = round_up(ceil_div(h->rows_per_launch, h->m_blks), 16);
-    }
-    // Two shared-memory rings: weight tiles (16 KB each) and activation tiles (tile_m x 128 B each).
-    // Weight ring depth: bytes in flight per SM just above the bandwidth-delay product (~80 KB x 148 SMs);
-    // a deeper ring only lengthens the memory queues, and with them every flag / partial round trip.
-    // Activation ring: deeper (its tiles are small at decode batch sizes), so that the consumer prologue's
-    // polls and fences run well ahead of the weight stream.
-    const int a_tile = h->tile_m * kTileK * 2;
-    const int max_smem = 227 * 1024 - kCtrlBytes - 1024;
-    int st = m.stages > 0 ? m.stages : std::max(4, ceil_div(80 * 1024, kWTileBytes));
-    st = std::max(2, std::min(st, kMaxStages));
-    int ast = std::max(st, std::min(kMaxStages, (32 * 1024) / a_tile));
-    while (st * kWTileBytes + ast * a_tile > max_smem && ast > st) --ast;
-    while (st * (kWTileBytes + a_tile) > max_smem && st > 2) --st;
-    ast = std::min(ast, std::max(st, (max_smem - st * kWTileBytes) / a_tile));
-    if (st * kWTileBytes + ast * a_tile > max_smem) ast = st;
-    h->stages = st;
-    h->a_stages = ast;
-    h->smem_bytes = static_cast<size_t>(st) * kWTileBytes + static_cast<size_t>(ast) * a_tile + kCtrlBytes + 1024;
-    h->grid = m.grid > 0 ? std::min(m.grid, h->num_sms) : h->num_sms;
-    const float s = (m.sm_split <= 0.0f) ? 1.0f : m.sm_split;
-    h->producer_ctas = h->grid;
-    if (m.kind == MLP_CTA_PIPELINED && h->L > 1 && s < 1.0f)
-        h->producer_ctas = std::min(h->grid, std::max(1, static_cast<int>(h->grid * s + 0.5f)));
+// ---------------------------------------------------------------------------------------------
+// The launch configuration: tile shape, ring depths, and per layer
+// the split of the contraction, how split tiles are reduced, and the ORDER of the tickets -- all of it
+// ends up in one unit table per layer that the kernel just walks.
+// ---------------------------------------------------------------------------------------------
 
-    // split-K per layer: the K-blocks of an output tile are cut into slices at h->bounds[l][0..split].
-    //  * a layer whose output is consumed inside the same launch stays tile-major (its tiles complete early,
-    //    one after the other) with <= 4 equal slices;
-    //  * a layer with more slices is handed out K-slice-major, so that its early units depend on the
-    //    producer's early tiles only; if it is the LAST layer of the launch its slices taper (guided
-    //    self-scheduling: each group of `tiles` units gets remaining_work / (2 * grid), within [4, cap]
-    //    K-blocks), so that the dynamic ticket ends the launch with small units and a short ragged tail.
-    // Candidates are ranked by a greedy list-scheduling model of the ticket order with +-8 % worker speeds.
+// Machine model of the list-scheduling simulation (microseconds, bytes per microsecond).  Fitted to
+// unit traces (mlp_pipe_cta_records) on B200: a CTA streams its share of HBM, an SM pulls at most
+// ~115 GB/s from L2, a gpu-scope fence costs the SM ~1 us of streaming.
+constexpr double kHbmBytesPerUs = 6.4e6;
+constexpr double kSmBytesPerUs = 115e3;
+constexpr double kSmFlopsPerUs = 13.0e6;
+constexpr double kDramLatencyUs = 1.3;
+constexpr double kSmStoreBytesPerUs = 45e3;       // st.global of fp32 partials while the rings stream
+constexpr double kUnitOverheadUs = 0.40;
+constexpr double kFenceUs = 0.90;
+constexpr double kPublishLatencyUs = 1.5;
+
+struct Planner {
+    mlp_pipe* h;
+    bool pipelined;
     int kb_total[kMaxLayers];
-    for (int l = 0; l < h->L; ++l) {
-        kb_total[l] = ceil_div(h->widths[l], kTileK);
-        h->tiles[l] = ceil_div(h->widths[l + 1], kTileN) * h->m_blks;
-    }
-    const bool pipelined = m.kind == MLP_CTA_PIPELINED;
-    const int kb_min = h->tile_m <= 32 ? 8 : h->tile_m <= 64 ? 16 : h->tile_m <= 128 ? 32 : 64;
-    const bool force_tile_major = (m.flags & (MLP_FLAG_TILE_MAJOR | MLP_FLAG_DEBUG_REVERSE)) != 0;
-    auto producer_in_launch = [&](int l) { return pipelined && l < h->L - 1; };
-    auto uniform = [&](int l, int sp) {
+    bool force_tile_major;
+
+    bool producer_in_launch(int l) const { return pipelined && l < h->L - 1; }
+    bool consumer_in_launch(int l) const { return pipelined && l > 0; }
+    size_t partial_bytes() const { return static_cast<size_t>(h->n_sub) * h->tile_m * kTileN * 4; }
+
+    std::vector<int> uniform(int l, int sp) const {
         sp = std::max(1, std::min(sp, kb_total[l]));
         std::vector<int> b(sp + 1);
         for (int i = 0; i <= sp; ++i) b[i] = static_cast<int>(static_cast<long long>(i) * kb_total[l] / sp);
         return b;
-    };
-    auto tapered = [&](int l, int cap) {
-        const int lo = std::max(4, kb_min / 2);
+    }
+    // guided self-scheduling: each group of `tiles` units gets remaining_work / (2 * grid), within [lo, cap]
+    std::vector<int> tapered(int l, int lo, int cap) const {
         std::vector<int> b{0};
         int rem = kb_total[l];
         while (rem > 0) {
@@ -214,94 +195,278 @@ void resolve(mlp_pipe* h) {
             rem -= sz;
         }
         return b;
-    };
-    auto ks_major_of = [&](int l, const std::vector<int>& b) {
-        return !force_tile_major && !producer_in_launch(l) && b.size() - 1 > 4;
-    };
-    // Costs in K-block equivalents (one K-block streams in ~0.36 us per SM), fitted to unit traces on cfg 1:
-    // every gpu-scope fence costs the SM ~1 us of streaming, and a unit of a split tile needs one (the
-    // arrival atomic), a consumer unit another one (the acquire of its ready counters).
-    const double unit_overhead = 1.0;
-    const double fence_cost = 2.5;
-    const double partial_cost = h->tile_m / 32.0;  // fp32 partial traffic per slice of a split tile
-    const double gather_cost = 0.55;               // per slice, paid once at the end of the launch by the last tile
-    const double publish_latency = 4.0;            // K-block equivalents from the last slice's MMA to a visible tile
-    auto makespan = [&](int lb, int le) {
-        std::vector<std::pair<double, int>> fin(h->grid);  // min-heap of (finish time, worker)
-        for (int i = 0; i < h->grid; ++i) fin[i] = {0.0, i};
+    }
+    int reduce_mode_for(int sp) const {
+        if (sp <= 1) return kReduceNone;
+        // the last arriver sums sp partials on ONE SM, kGather slices x 16 token columns per dependent round
+        // trip: fine for decode-sized tiles (<= 2 trips), a long serial tail otherwise
+        const int trips = h->n_sub * (h->tile_m / 16) * ((sp + kGather - 1) / kGather);
+        return trips <= 2 ? kReduceLastArriver : kReduceUnits;
+    }
+    // token columns per reduce unit: about one reduce unit per CTA and layer, at least 16 columns
+    int reduce_cols(int l) const {
+        const int chunks = std::max(1, std::min(h->tile_m / 16, (h->grid + h->tiles[l] - 1) / h->tiles[l]));
+        return ((h->tile_m + chunks - 1) / chunks + 15) / 16 * 16;
+    }
+
+    // Ticket order of layer l for slice boundaries b.
+    //  * last-arriver layers: tile-major while the output is consumed inside the launch and the split is small
+    //    (tiles complete early, one after the other), K-slice-major otherwise (early units depend on the
+    //    producer's early tiles only);
+    //  * reduce-unit layers: a producer stays tile-major and the reduce units of a tile follow its slices
+    //    about one wave of tickets later (so its partials have normally arrived when the unit is drawn, and
+    //    tiles still complete progressively); the last layer of a launch is K-slice-major with all reduce
+    //    units at the end.
+    void build_table(int l, const std::vector<int>& b, std::vector<UnitDesc>& out, int& mode, int& ready_inc) const {
+        const int sp = static_cast<int>(b.size()) - 1, tiles = h->tiles[l];
+        mode = reduce_mode_for(sp);
+        ready_inc = 1;
+        out.clear();
+        auto mma = [&](int tile, int ks) {
+            UnitDesc d;
+            d.tile = static_cast<uint16_t>(tile);
+            d.kind = kUnitMma;
+            d.ks = static_cast<uint8_t>(ks);
+            d.a = static_cast<uint16_t>(b[ks]);
+            d.b = static_cast<uint16_t>(b[ks + 1]);
+            out.push_back(d);
+        };
+        const bool reverse = (h->mode.flags & MLP_FLAG_DEBUG_REVERSE) && (l == 0 || !pipelined);
+        bool ksm;
+        if (mode == kReduceUnits) ksm = !force_tile_major && !producer_in_launch(l) && consumer_in_launch(l);
+        else ksm = !force_tile_major && !producer_in_launch(l) && sp > 4;
+        if (ksm) {
+            for (int ks = 0; ks < sp; ++ks)
+                for (int t = 0; t < tiles; ++t) mma(t, ks);
+        } else {
+            for (int t = 0; t < tiles; ++t)
+                for (int ks = 0; ks < sp; ++ks) mma(t, ks);
+        }
+        if (reverse) std::reverse(out.begin(), out.end());
+        if (mode != kReduceUnits) return;
+        const int cols = reduce_cols(l);
+        const int chunks = (h->tile_m + cols - 1) / cols;
+        ready_inc = chunks;
+        auto red = [&](int tile, int c) {
+            UnitDesc d;
+            d.tile = static_cast<uint16_t>(tile);
+            d.kind = kUnitReduce;
+            d.ks = 0;
+            d.a = static_cast<uint16_t>(c * cols);
+            d.b = static_cast<uint16_t>(std::min(h->tile_m, (c + 1) * cols));
+            return d;
+        };
+        if (ksm || reverse) {
+            for (int t = 0; t < tiles; ++t)
+                for (int c = 0; c < chunks; ++c) out.push_back(red(t, c));
+            return;
+        }
+        // tile-major: interleave.  Tile t's last slice has ticket (t + 1) sp - 1; its reduce units go after
+        // ticket (t + 1) sp - 1 + delay of the MMA sequence.
+        const int delay = h->grid + h->grid / 4;
+        std::vector<UnitDesc> merged;
+        merged.reserve(out.size() + static_cast<size_t>(tiles) * chunks);
+        int next_red = 0;
+        for (int i = 0; i < static_cast<int>(out.size()); ++i) {
+            merged.push_back(out[i]);
+            while (next_red < tiles && (next_red + 1) * sp - 1 + delay <= i) {
+                for (int c = 0; c < chunks; ++c) merged.push_back(red(next_red, c));
+                ++next_red;
+            }
+        }
+        for (; next_red < tiles; ++next_red)
+            for (int c = 0; c < chunks; ++c) merged.push_back(red(next_red, c));
+        out.swap(merged);
+    }
+
+    void build_all() const {
+        for (int l = 0; l < h->L; ++l) build_table(l, h->bounds[l], h->table[l], h->reduce_mode[l], h->ready_inc[l]);
+    }
+
+    // Greedy list scheduling of the tables of layers [lb, le) in ticket order on `grid` workers.
+    double makespan(int lb, int le) const {
+        const int G = h->grid, R = h->n_sub, tm = h->tile_m;
+        const double w_bytes = R * static_cast<double>(kWTileBytes), a_bytes = tm * 128.0;
+        size_t mma_units = 0;
+        for (int l = lb; l < le; ++l) mma_units += static_cast<size_t>(h->tiles[l]) * (h->bounds[l].size() - 1);
+        const int active = static_cast<int>(std::min<size_t>(G, std::max<size_t>(1, mma_units)));  // CTAs that share HBM
+        // one SM streams from DRAM at most its ring of outstanding weight bytes per DRAM latency
+        const double t_kb = std::max({w_bytes / (kHbmBytesPerUs / active), w_bytes / (h->stages * w_bytes / kDramLatencyUs),
+                                      (w_bytes + a_bytes) / kSmBytesPerUs, 2.0 * R * kTileN * tm * kTileK / kSmFlopsPerUs});
+        // a dependent global round trip queues behind the SM's own ring of TMA requests, which drains at the
+        // rate the main loop consumes it
+        const double rtt = 0.6 + 0.5 * (h->stages * w_bytes + h->a_stages * a_bytes) / ((w_bytes + a_bytes) / t_kb);
+        const double part_us = partial_bytes() / kSmStoreBytesPerUs;
+        const double epi_us = R * tm * 0.004 + 0.3;  // act + convert + transpose of one accumulator
+        // sum of `cols` token columns over sp partials by ONE CTA: kGather slices x 16 columns per round trip
+        auto gather_us = [&](int sp, int cols) {
+            const int trips = R * ((cols + 15) / 16) * ((sp + kGather - 1) / kGather);
+            return trips * rtt + static_cast<double>(sp) * R * cols * kTileN * 4 / kSmBytesPerUs;
+        };
+        std::vector<std::pair<double, int>> fin(G);  // min-heap of (finish time, worker)
+        for (int i = 0; i < G; ++i) fin[i] = {0.0, i};
         auto cmp = [](const std::pair<double, int>& x, const std::pair<double, int>& y) { return x.first > y.first; };
         double end = 0.0;
-        std::vector<double> done_prev, done_cur;  // per output tile: when it is published
+        std::vector<double> done_prev, done_cur, part_done;
+        std::vector<int> arrived;
         for (int l = lb; l < le; ++l) {
-            const std::vector<int>& b = h->bounds[l];
-            const int sp = static_cast<int>(b.size()) - 1, tiles = h->tiles[l];
+            const std::vector<UnitDesc>& tb = h->table[l];
+            const int sp = static_cast<int>(h->bounds[l].size()) - 1, tiles = h->tiles[l];
             const int n_blks = tiles / h->m_blks;
             const int n_blks_prev = l > lb ? h->tiles[l - 1] / h->m_blks : 0;
-            const bool ksm = ks_major_of(l, b);
+            const int mode = h->reduce_mode[l];
             done_cur.assign(tiles, 0.0);
-            for (int u = 0; u < tiles * sp; ++u) {
-                const int ks = ksm ? u / tiles : u % sp;
-                const int tile = ksm ? u % tiles : u / sp;
+            part_done.assign(tiles, 0.0);
+            arrived.assign(tiles, 0);
+            for (const UnitDesc& d : tb) {
                 std::pop_heap(fin.begin(), fin.end(), cmp);
                 const double speed = 1.0 + 0.08 * (((fin.back().second * 37) % 11) - 5) / 5.0;
-                double start = fin.back().first;
-                if (l > lb) {  // the consumer prologue waits for the producer tiles under its K range
-                    const int m_blk = tile / n_blks;
-                    for (int j = (b[ks] * kTileK) / kTileN; j <= ((b[ks + 1] - 1) * kTileK) / kTileN && j < n_blks_prev; ++j)
-                        start = std::max(start, done_prev[m_blk * n_blks_prev + j]);
+                double start = fin.back().first, busy, done;
+                if (d.kind == kUnitMma) {
+                    if (l > lb) {  // the consumer prologue waits for the producer tiles under its K range
+                        const int m_blk = d.tile / n_blks;
+                        const int tn = kTileN * R;
+                        for (int j = (d.a * kTileK) / tn; j <= ((d.b - 1) * kTileK) / tn && j < n_blks_prev; ++j)
+                            start = std::max(start, done_prev[m_blk * n_blks_prev + j]);
+                    }
+                    double ovh = kUnitOverheadUs + (l > lb && pipelined ? kFenceUs : 0.0);
+                    if (sp > 1) ovh += kFenceUs + 0.5 * part_us;
+                    busy = ((d.b - d.a) * t_kb + ovh) * speed;
+                    done = start + busy;
+                    double fin_t = done;  // when this unit's share of the layer's output is in memory
+                    if (sp == 1) {
+                        fin_t = done + epi_us;
+                        done_cur[d.tile] = fin_t + kPublishLatencyUs;
+                    } else {
+                        part_done[d.tile] = std::max(part_done[d.tile], done + part_us + rtt);
+                        if (mode == kReduceLastArriver && ++arrived[d.tile] == sp) {
+                            fin_t = part_done[d.tile] + gather_us(sp, tm);
+                            done_cur[d.tile] = fin_t + kPublishLatencyUs;
+                        }
+                    }
+                    end = std::max(end, fin_t);
+                } else {
+                    const double g_us = gather_us(sp, d.b - d.a);
+                    start = std::max(start, part_done[d.tile]);
+                    busy = 0.35 * g_us * speed;  // epilogue warps only: the main loop of the next unit overlaps
+                    done = start + g_us;
+                    done_cur[d.tile] = std::max(done_cur[d.tile], done + kPublishLatencyUs);
+                    end = std::max(end, done);
                 }
-                const double ovh = unit_overhead + (sp > 1 ? partial_cost + fence_cost : 0.0) + (l > lb && pipelined ? fence_cost : 0.0);
-                const double t = start + (b[ks + 1] - b[ks] + ovh) * speed;
-                fin.back().first = t;
+                fin.back().first = start + busy;
                 std::push_heap(fin.begin(), fin.end(), cmp);
-                done_cur[tile] = std::max(done_cur[tile], t + publish_latency);
-                end = std::max(end, t);
             }
             done_prev.swap(done_cur);
-            if (l == le - 1 && sp > 1) end += gather_cost * sp;
         }
         return end;
-    };
+    }
+};
+
+void resolve(mlp_pipe* h) {
+    const mlp_mode& m = h->mode;
+    h->rows_per_launch = m.kind == MLP_MICROBATCH ? h->M / m.chunks : h->M;
+    if (m.tile_m > 0) {
+        h->tile_m = m.tile_m;
+        h->m_blks = ceil_div(h->rows_per_launch, h->tile_m);
+    } else {
+        h->m_blks = ceil_div(h->rows_per_launch, 256);
+        h->tile_m = round_up(ceil_div(h->rows_per_launch, h->m_blks), 16);
+    }
+    // Weight rows per unit: 256 (two MMAs per K step that share the activation tile) once the activation
+    // tile is large enough for its L2 traffic to matter and two accumulators still fit twice into TMEM.
+    if (m.tile_n == 2 * kTileN) h->n_sub = 2;
+    else if (m.tile_n == kTileN) h->n_sub = 1;
+    else h->n_sub = (h->tile_m >= 96 && h->tile_m <= 128) ? 2 : 1;
+    h->acc_stages = std::max(1, std::min(kMaxAccStages, 512 / (h->n_sub * h->tile_m)));
+    // Shared-memory rings: weight tiles (16 KB x n_sub each) and activation tiles (tile_m x 128 B each).
+    // Weight ring depth: bytes in flight per SM just above the bandwidth-delay product (~80 KB x 148 SMs);
+    // a deeper ring only lengthens the memory queues, and with them every flag / partial round trip.
+    // Activation ring: deeper (its tiles are small at decode batch sizes), so that the consumer prologue's
+    // polls and fences run well ahead of the weight stream.
+    const int w_tile = h->n_sub * kWTileBytes;
+    const int a_tile = h->tile_m * kTileK * 2;
+    const int max_smem = 227 * 1024 - kCtrlBytes - 1024 - kStageBytes;
+    int st = m.stages > 0 ? m.stages : std::max(4, ceil_div(80 * 1024, w_tile));
+    st = std::max(2, std::min(st, kMaxStages));
+    int ast = std::max(st, std::min(kMaxStages, (32 * 1024) / a_tile));
+    while (st * w_tile + ast * a_tile > max_smem && ast > st) --ast;
+    while (st * (w_tile + a_tile) > max_smem && st > 2) --st;
+    ast = std::min(ast, std::max(st, (max_smem - st * w_tile) / a_tile));
+    if (st * w_tile + ast * a_tile > max_smem) ast = st;
+    h->stages = st;
+    h->a_stages = ast;
+    h->smem_bytes = static_cast<size_t>(st) * w_tile + static_cast<size_t>(ast) * a_tile + kStageBytes + kCtrlBytes + 1024;
+    h->grid = m.grid > 0 ? std::min(m.grid, h->num_sms) : h->num_sms;
+    const float s = (m.sm_split <= 0.0f) ? 1.0f : m.sm_split;
+    h->producer_ctas = h->grid;
+    if (m.kind == MLP_CTA_PIPELINED && h->L > 1 && s < 1.0f)
+        h->producer_ctas = std::min(h->grid, std::max(1, static_cast<int>(h->grid * s + 0.5f)));
+
+    Planner pl;
+    pl.h = h;
+    pl.pipelined = m.kind == MLP_CTA_PIPELINED;
+    pl.force_tile_major = (m.flags & (MLP_FLAG_TILE_MAJOR | MLP_FLAG_DEBUG_REVERSE)) != 0;
+    for (int l = 0; l < h->L; ++l) {
+        pl.kb_total[l] = ceil_div(h->widths[l], kTileK);
+        h->tiles[l] = ceil_div(h->widths[l + 1], kTileN * h->n_sub) * h->m_blks;
+    }
+    // smallest slice worth a unit: the fp32 partial of a split tile should stay below ~1/8 of the operand
+    // bytes the slice streams
+    const int kb_min = std::max(h->tile_m <= 32 ? 8 : 16, static_cast<int>(8 * pl.partial_bytes() / (w_tile + a_tile)) / 4 * 4);
+    const int kb_floor = std::max(4, kb_min / 2);
     bool fixed[kMaxLayers];
     for (int l = 0; l < h->L; ++l) {
         int sp = m.split_k_layer[l] > 0 ? m.split_k_layer[l] : m.split_k;
         fixed[l] = sp > 0;
         if (sp <= 0) {
-            sp = std::min(ceil_div(3 * h->grid, h->tiles[l]), std::max(1, kb_total[l] / kb_min));
-            if (producer_in_launch(l)) sp = std::min(sp, 4);
+            sp = std::min(ceil_div(3 * h->grid, h->tiles[l]), std::max(1, pl.kb_total[l] / kb_min));
+            if (pl.producer_in_launch(l) && pl.reduce_mode_for(sp) == kReduceLastArriver) sp = std::min(sp, 4);
         }
-        h->bounds[l] = uniform(l, sp);
+        h->bounds[l] = pl.uniform(l, std::min(sp, 255));
     }
+    pl.build_all();
+    // Candidates are ranked by the simulated makespan of the actual tables; coordinate descent over the layers.
     auto refine = [&](int lb, int le) {
         for (int pass = 0; pass < 2; ++pass)
             for (int l = le - 1; l >= lb; --l) {
                 if (fixed[l]) continue;
                 std::vector<std::vector<int>> cand;
-                const int kb_floor = std::max(4, kb_min / 2);
-                int s_max = std::max(1, std::min(64, kb_total[l] / kb_floor));
-                if (producer_in_launch(l)) s_max = std::min(s_max, 4);
-                for (int c = 1; c <= s_max; ++c) cand.push_back(uniform(l, c));
-                if (l == le - 1 && !force_tile_major && !producer_in_launch(l))
+                const int s_max = std::max(1, std::min(64, pl.kb_total[l] / kb_floor));
+                for (int c = 1; c <= s_max; ++c) {
+                    if (pl.producer_in_launch(l) && c > 4 && pl.reduce_mode_for(c) == kReduceLastArriver) continue;
+                    cand.push_back(pl.uniform(l, c));
+                }
+                if (l == le - 1 && !pl.force_tile_major && !pl.producer_in_launch(l))
                     for (int cap : {2 * kb_floor, 3 * kb_floor, 4 * kb_floor, 6 * kb_floor, 8 * kb_floor}) {
-                        std::vector<int> t = tapered(l, cap);
+                        std::vector<int> t = pl.tapered(l, kb_floor, cap);
                         if (t.size() - 1 > 4 && t.size() - 1 <= 64) cand.push_back(t);
                     }
                 std::vector<int> best = h->bounds[l];
-                double best_t = makespan(lb, le);
+                pl.build_table(l, best, h->table[l], h->reduce_mode[l], h->ready_inc[l]);
+                double best_t = pl.makespan(lb, le);
                 for (auto& c : cand) {
                     h->bounds[l] = c;
-                    const double t = makespan(lb, le);
+                    pl.build_table(l, c, h->table[l], h->reduce_mode[l], h->ready_inc[l]);
+                    const double t = pl.makespan(lb, le);
                     if (t < best_t * 0.995) { best_t = t; best = c; }
                 }
                 h->bounds[l] = best;
+                pl.build_table(l, best, h->table[l], h->reduce_mode[l], h->ready_inc[l]);
             }
     };
-    if (pipelined) refine(0, h->L);
+    if (pl.pipelined) refine(0, h->L);
     else
         for (int l = 0; l < h->L; ++l) refine(l, l + 1);
-    for (int l = 0; l < h->L; ++l) {
-        h->split[l] = static_cast<int>(h->bounds[l].size()) - 1;
-        h->ks_major[l] = ks_major_of(l, h->bounds[l]) ? 1 : 0;
+    for (int l = 0; l < h->L; ++l) h->split[l] = static_cast<int>(h->bounds[l].size()) - 1;
+    if (getenv("MLP_PIPE_DEBUG")) {
+        fprintf(stderr, "[mlp_pipe] M=%d tile %dx%d stages %d/%d acc %d grid %d mode %d: model %.1f us\n", h->M, kTileN * h->n_sub,
+                h->tile_m, h->stages, h->a_stages, h->acc_stages, h->grid, m.kind, pl.pipelined ? pl.makespan(0, h->L) : -1.0);
+        for (int l = 0; l < h->L; ++l) {
+            fprintf(stderr, "[mlp_pipe]  layer %d: tiles %d split %d reduce_mode %d ready_inc %d units %zu bounds", l, h->tiles[l], h->split[l],
+                    h->reduce_mode[l], h->ready_inc[l], h->table[l].size());
+            for (int b : h->bounds[l]) fprintf(stderr, " %d", b);
+            fprintf(stderr, "%s\n", pl.pipelined ? "" : (std::string("  model ") + std::to_string(pl.makespan(l, l + 1))).c_str());
+        }
     }
 }
 
@@ -313,13 +478,14 @@ int build_base_params(mlp_pipe* h) {
         Lp.K = h->widths[l];
         Lp.N = h->widths[l + 1];
         Lp.kb_total = ceil_div(Lp.K, kTileK);
-        Lp.n_blks = ceil_div(Lp.N, kTileN);
+        Lp.n_blks = ceil_div(Lp.N, kTileN * h->n_sub);
         Lp.split = h->split[l];
-        Lp.units = h->tiles[l] * h->split[l];
+        Lp.units = static_cast<int>(h->table[l].size());
         Lp.act = l < h->L - 1 ? h->act : kActNone;
         Lp.publish = l < h->L - 1 ? 1 : 0;
-        Lp.ks_major = h->ks_major[l];
-        Lp.kb_bounds = h->d_bounds[l];
+        Lp.reduce_mode = h->reduce_mode[l];
+        Lp.ready_inc = h->ready_inc[l];
+        Lp.table = h->d_table[l];
         Lp.out = l < h->L - 1 ? h->H[l] : nullptr;  // last layer: caller's Y, patched per run
         Lp.ws = h->ws[l];
         Lp.ticket = h->ticket[l];
@@ -334,7 +500,15 @@ int build_base_params(mlp_pipe* h) {
     P.m_blks = h->m_blks;
     P.stages = h->stages;
     P.a_stages = h->a_stages;
-    P.acc_stages = std::min(kMaxAccStages, 512 / h->tile_m);
+    P.n_sub = h->n_sub;
+    {   // the next ticket is drawn ~2.5 loaded round trips (ticket atomic, table entry, ready counters) before
+        // the weight loader runs out of K-blocks
+        const double w_bytes = h->n_sub * static_cast<double>(kWTileBytes), a_bytes = h->tile_m * 128.0;
+        const double t_kb = std::max(w_bytes / (kHbmBytesPerUs / h->grid), (w_bytes + a_bytes) / kSmBytesPerUs);
+        const double rtt = 0.6 + 0.5 * (h->stages * w_bytes + h->a_stages * a_bytes) / ((w_bytes + a_bytes) / t_kb);
+        P.claim_ahead = std::max(2, static_cast<int>((2.5 * rtt + 0.5) / t_kb + 0.5));
+    }
+    P.acc_stages = h->acc_stages;
     P.w_group = std::max(1, std::min(h->mode.w_group > 0 ? h->mode.w_group : 1, h->stages));
     P.flags = h->mode.flags;
     P.status = h->status;
@@ -456,13 +630,12 @@ int create_impl(mlp_pipe** out, int M, int L, const int* widths, int dtype, int 
         }
     }
     for (int l = 0; l < L; ++l) {
-        std::vector<uint16_t> b16(h->bounds[l].begin(), h->bounds[l].end());
-        CREATE_TRY(cudaMalloc(&h->d_bounds[l], b16.size() * sizeof(uint16_t)));
-        CREATE_TRY(cudaMemcpy(h->d_bounds[l], b16.data(), b16.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
+        CREATE_TRY(cudaMalloc(&h->d_table[l], h->table[l].size() * sizeof(UnitDesc)));
+        CREATE_TRY(cudaMemcpy(h->d_table[l], h->table[l].data(), h->table[l].size() * sizeof(UnitDesc), cudaMemcpyHostToDevice));
     }
     for (int l = 0; l < L; ++l)
         if (h->split[l] > 1)
-            CREATE_TRY(cudaMalloc(&h->ws[l], static_cast<size_t>(h->tiles[l]) * h->split[l] * h->tile_m * kTileN * sizeof(float)));
+            CREATE_TRY(cudaMalloc(&h->ws[l], static_cast<size_t>(h->tiles[l]) * h->split[l] * h->n_sub * h->tile_m * kTileN * sizeof(float)));
     CREATE_TRY(cudaMalloc(&h->epoch, kMaxLayers * sizeof(unsigned long long)));
     CREATE_TRY(cudaMalloc(&h->status, sizeof(uint32_t)));
     CREATE_TRY(cudaMalloc(&h->stats, sizeof(CtaStats) * kMaxLayers * h->grid));
@@ -508,7 +681,7 @@ int run_impl(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStre
     KernelParams P = h->base;
     if ((rc = lookup_tmap(h, h->cache_x, &h->cache_x_next, X, h->M, h->widths[0], h->tile_m, &P.tm_a[0]))) return rc;
     for (int l = 0; l < h->L; ++l)
-        if ((rc = lookup_tmap(h, h->cache_w[l], &h->cache_w_next[l], W[l], h->widths[l + 1], h->widths[l], kTileN, &P.tm_w[l])))
+        if ((rc = lookup_tmap(h, h->cache_w[l], &h->cache_w_next[l], W[l], h->widths[l + 1], h->widths[l], kTileN * h->n_sub, &P.tm_w[l])))
             return rc;
     P.layer[h->L - 1].out = static_cast<__nv_bfloat16*>(Y);
 
@@ -648,10 +821,12 @@ int mlp_pipe_stats(mlp_pipe* h, mlp_stats* out, size_t bytes) {
     st.grid = h->grid;
     st.stages = h->stages;
     st.tile_m = h->tile_m;
+    st.tile_n = kTileN * h->n_sub;
     st.producer_ctas = h->producer_ctas;
     for (int l = 0; l < h->L; ++l) {
         st.split_k[l] = h->split[l];
-        st.units[l] = h->tiles[l] * h->split[l];
+        st.units[l] = static_cast<int>(h->table[l].size());
+        st.reduce_mode[l] = h->reduce_mode[l];
     }
     CUDA_TRY(h, cudaMemcpy(&st.status, h->status, sizeof(uint32_t), cudaMemcpyDeviceToHost));
     unsigned long long ep[kMaxLayers];
@@ -685,7 +860,7 @@ int mlp_pipe_stats(mlp_pipe* h, mlp_stats* out, size_t bytes) {
         ok = ok && tk[0] == static_cast<uint32_t>(e * static_cast<unsigned long long>(st.units[l] + arrivals));
         for (int t = 0; t < h->tiles[l] && ok; ++t) {
             ok = ok && ar[t] == (h->split[l] > 1 ? static_cast<uint32_t>(e * h->split[l]) : 0u);
-            ok = ok && rd[t] == (l < h->L - 1 ? static_cast<uint32_t>(e) : 0u);
+            ok = ok && rd[t] == (l < h->L - 1 ? static_cast<uint32_t>(e * h->ready_inc[l]) : 0u);
         }
     }
     st.ready_ok = ok ? 1u : 0u;
@@ -715,7 +890,7 @@ void mlp_pipe_destroy(mlp_pipe* h) {
     for (int l = 0; l < kMaxLayers; ++l) {
         if (h->H[l]) cudaFree(h->H[l]);
         if (h->ws[l]) cudaFree(h->ws[l]);
-        if (h->d_bounds[l]) cudaFree(h->d_bounds[l]);
+        if (h->d_table[l]) cudaFree(h->d_table[l]);
         if (h->stage_W[l]) cudaFree(h->stage_W[l]);
     }
     if (h->counters) cudaFree(h->counters);
