@@ -204,6 +204,34 @@ typedef struct {
 } mlp_cta_record;
 int mlp_pipe_cta_records(mlp_pipe* h, int cls, mlp_cta_record* out, int max_records, int* n_out);
 
+/*
+ * The launch plan the library would use for this problem on a device with `num_sms` SMs, WITHOUT touching
+ * a device (host logic only; works on a CPU-only box): tile shape, ring depths, per-layer split of the
+ * contraction, how split tiles are summed, and the planner's latency estimate.  The ticket order itself
+ * (step a1: the order in which work is handed out is the scheduling knob) is returned by
+ * mlp_pipe_plan_units: unit i of `layer` is what ticket i of that layer executes.
+ */
+typedef struct {
+    int tile_m, tile_n, m_blks, stages, a_stages, acc_stages, grid, producer_ctas, smem_bytes;
+    int tiles[MLP_MAX_LAYERS];       /* output tiles per layer (m_blks x ceil(N / tile_n))               */
+    int split_k[MLP_MAX_LAYERS];     /* K-slices per output tile                                          */
+    int reduce_mode[MLP_MAX_LAYERS]; /* 0 not split, 1 last-arriving slice sums, 2 reduce units           */
+    int ready_inc[MLP_MAX_LAYERS];   /* ready-counter increments per tile and run                         */
+    int units[MLP_MAX_LAYERS];       /* tickets per layer                                                 */
+    double model_us;                 /* planner's estimate of one run (device time, microseconds)         */
+} mlp_plan;
+typedef struct {
+    uint16_t tile;     /* m_blk * n_blks + n_blk                                                          */
+    uint8_t kind;      /* 0 = MMA unit over K-blocks [begin, end) (64 elements each); 1 = reduce unit over
+                          token columns [begin, end) of the tile                                          */
+    uint8_t k_slice;   /* MMA unit: index of its K-slice                                                  */
+    uint16_t begin, end;
+} mlp_unit;
+int mlp_pipe_plan(int M, int n_layers, const int* widths, const mlp_mode* mode, int num_sms, mlp_plan* out);
+/* Copies min(max_units, n) units of `layer` to out; *n_out = n, the number of tickets of that layer. */
+int mlp_pipe_plan_units(int M, int n_layers, const int* widths, const mlp_mode* mode, int num_sms, int layer,
+                        mlp_unit* out, int max_units, int* n_out);
+
 /* Free everything the handle owns (synchronises the device).  NULL is ignored. */
 void mlp_pipe_destroy(mlp_pipe* h);
 

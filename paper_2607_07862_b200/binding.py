@@ -25,7 +25,7 @@ MLP_FLAG_TILE_MAJOR, MLP_FLAG_DEBUG_DELAY, MLP_FLAG_DEBUG_REVERSE, MLP_FLAG_NO_W
 EXPORTS = [
     "mlp_pipe_create", "mlp_pipe_create_chain", "mlp_pipe_run", "mlp_pipe_run_chain", "mlp_pipe_run_host",
     "mlp_pipe_hidden", "mlp_pipe_poison_hidden", "mlp_pipe_stats", "mlp_pipe_destroy", "mlp_status_string",
-    "mlp_pipe_last_error", "mlp_pipe_version", "mlp_pipe_cta_records",
+    "mlp_pipe_last_error", "mlp_pipe_version", "mlp_pipe_cta_records", "mlp_pipe_plan", "mlp_pipe_plan_units",
 ]
 
 
@@ -58,6 +58,22 @@ class mlp_cta_record(ctypes.Structure):
         ("ts", ctypes.c_uint64 * 8), ("wait", ctypes.c_uint64 * 8), ("units", ctypes.c_uint32 * MLP_MAX_LAYERS),
         ("unit_ts", (ctypes.c_uint64 * 4) * 12), ("unit_id", ctypes.c_uint32 * 12),
     ]
+
+
+class mlp_plan(ctypes.Structure):
+    _fields_ = [
+        ("tile_m", ctypes.c_int), ("tile_n", ctypes.c_int), ("m_blks", ctypes.c_int), ("stages", ctypes.c_int),
+        ("a_stages", ctypes.c_int), ("acc_stages", ctypes.c_int), ("grid", ctypes.c_int), ("producer_ctas", ctypes.c_int),
+        ("smem_bytes", ctypes.c_int),
+        ("tiles", ctypes.c_int * MLP_MAX_LAYERS), ("split_k", ctypes.c_int * MLP_MAX_LAYERS),
+        ("reduce_mode", ctypes.c_int * MLP_MAX_LAYERS), ("ready_inc", ctypes.c_int * MLP_MAX_LAYERS),
+        ("units", ctypes.c_int * MLP_MAX_LAYERS), ("model_us", ctypes.c_double),
+    ]
+
+
+class mlp_unit(ctypes.Structure):
+    _fields_ = [("tile", ctypes.c_uint16), ("kind", ctypes.c_uint8), ("k_slice", ctypes.c_uint8),
+                ("begin", ctypes.c_uint16), ("end", ctypes.c_uint16)]
 
 
 _lib = None
@@ -98,6 +114,11 @@ def load(build_if_missing: bool = True):
     lib.mlp_pipe_stats.argtypes = [vp, ctypes.POINTER(mlp_stats), ctypes.c_size_t]
     lib.mlp_pipe_cta_records.restype = ci
     lib.mlp_pipe_cta_records.argtypes = [vp, ci, ctypes.POINTER(mlp_cta_record), ci, ctypes.POINTER(ci)]
+    lib.mlp_pipe_plan.restype = ci
+    lib.mlp_pipe_plan.argtypes = [ci, ci, ctypes.POINTER(ci), ctypes.POINTER(mlp_mode), ci, ctypes.POINTER(mlp_plan)]
+    lib.mlp_pipe_plan_units.restype = ci
+    lib.mlp_pipe_plan_units.argtypes = [ci, ci, ctypes.POINTER(ci), ctypes.POINTER(mlp_mode), ci, ci, ctypes.POINTER(mlp_unit), ci,
+                                        ctypes.POINTER(ci)]
     lib.mlp_pipe_destroy.restype = None
     lib.mlp_pipe_destroy.argtypes = [vp]
     lib.mlp_status_string.restype = ctypes.c_char_p
@@ -241,6 +262,23 @@ class _RawCudaBuffer:
 
     def __init__(self, ptr: int, nbytes: int):
         self.__cuda_array_interface__ = {"shape": (nbytes,), "typestr": "|u1", "data": (ptr, False), "version": 2}
+
+
+def plan(M: int, widths: Sequence[int], mode: Optional[mlp_mode] = None, num_sms: int = 148):
+    """Host-only: the launch plan for this problem (no device needed).  Returns (mlp_plan, [units of layer 0, ...])."""
+    lib = load()
+    L = len(widths) - 1
+    w = (ctypes.c_int * (L + 1))(*[int(x) for x in widths])
+    mp = ctypes.byref(mode) if mode is not None else None
+    out = mlp_plan()
+    _check(lib.mlp_pipe_plan(int(M), L, w, mp, int(num_sms), ctypes.byref(out)))
+    tables = []
+    for l in range(L):
+        n = ctypes.c_int()
+        arr = (mlp_unit * out.units[l])()
+        _check(lib.mlp_pipe_plan_units(int(M), L, w, mp, int(num_sms), l, arr, out.units[l], ctypes.byref(n)))
+        tables.append([(u.tile, u.kind, u.k_slice, u.begin, u.end) for u in arr])
+    return out, tables
 
 
 def version() -> str:

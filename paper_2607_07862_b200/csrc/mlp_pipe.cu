@@ -52,6 +52,7 @@ struct mlp_pipe {
     std::vector<UnitDesc> table[kMaxLayers];   // ticket -> unit
     UnitDesc* d_table[kMaxLayers] = {nullptr};  // the same on the device
     int tiles[kMaxLayers] = {0};
+    double model_us = 0.0;  // the planner's estimate of the launch(es)
     // device memory owned by the handle
     __nv_bfloat16* H[kMaxLayers] = {nullptr};  // H[l] = output of layer l, l < L-1
     float* ws[kMaxLayers] = {nullptr};
@@ -158,13 +159,13 @@ int validate_mode(const mlp_mode& m, int M) {
 // Machine model of the list-scheduling simulation (microseconds, bytes per microsecond).  Fitted to
 // unit traces (mlp_pipe_cta_records) on B200: a CTA streams its share of HBM, an SM pulls at most
 // ~115 GB/s from L2, a gpu-scope fence costs the SM ~1 us of streaming.
-constexpr double kHbmBytesPerUs = 6.4e6;
+constexpr double kHbmBytesPerUs = 6.23e6;
 constexpr double kSmBytesPerUs = 115e3;
 constexpr double kSmFlopsPerUs = 13.0e6;
 constexpr double kDramLatencyUs = 1.3;
 constexpr double kSmStoreBytesPerUs = 45e3;       // st.global of fp32 partials while the rings stream
-constexpr double kUnitOverheadUs = 0.40;
-constexpr double kFenceUs = 0.90;
+constexpr double kUnitOverheadUs = 0.15;
+constexpr double kFenceUs = 0.10;
 constexpr double kPublishLatencyUs = 1.5;
 
 struct Planner {
@@ -458,6 +459,10 @@ void resolve(mlp_pipe* h) {
     else
         for (int l = 0; l < h->L; ++l) refine(l, l + 1);
     for (int l = 0; l < h->L; ++l) h->split[l] = static_cast<int>(h->bounds[l].size()) - 1;
+    h->model_us = 0.0;
+    if (pl.pipelined) h->model_us = pl.makespan(0, h->L);
+    else
+        for (int l = 0; l < h->L; ++l) h->model_us += pl.makespan(l, l + 1) * (m.kind == MLP_MICROBATCH ? m.chunks : 1);
     if (getenv("MLP_PIPE_DEBUG")) {
         fprintf(stderr, "[mlp_pipe] M=%d tile %dx%d stages %d/%d acc %d grid %d mode %d: model %.1f us\n", h->M, kTileN * h->n_sub,
                 h->tile_m, h->stages, h->a_stages, h->acc_stages, h->grid, m.kind, pl.pipelined ? pl.makespan(0, h->L) : -1.0);
@@ -905,6 +910,75 @@ void mlp_pipe_destroy(mlp_pipe* h) {
     for (auto e : h->ev_done)
         if (e) cudaEventDestroy(e);
     delete h;
+}
+
+int mlp_pipe_plan(int M, int n_layers, const int* widths, const mlp_mode* mode, int num_sms, mlp_plan* out) {
+    if (!out || !widths || n_layers < 1 || n_layers > kMaxLayers || M < 1 || num_sms < 1) return MLP_ERR_INVALID;
+    for (int l = 0; l <= n_layers; ++l)
+        if (widths[l] < 8 || widths[l] % 8 != 0) return MLP_ERR_INVALID;
+    mlp_mode m{};
+    if (mode) m = *mode;
+    else m.kind = MLP_CTA_PIPELINED;
+    int rc = validate_mode(m, M);
+    if (rc) return rc;
+    mlp_pipe h;
+    h.M = M;
+    h.L = n_layers;
+    for (int l = 0; l <= n_layers; ++l) h.widths[l] = widths[l];
+    h.mode = m;
+    h.num_sms = num_sms;
+    resolve(&h);
+    memset(out, 0, sizeof *out);
+    out->tile_m = h.tile_m;
+    out->tile_n = kTileN * h.n_sub;
+    out->m_blks = h.m_blks;
+    out->stages = h.stages;
+    out->a_stages = h.a_stages;
+    out->acc_stages = h.acc_stages;
+    out->grid = h.grid;
+    out->producer_ctas = h.producer_ctas;
+    out->smem_bytes = static_cast<int>(h.smem_bytes);
+    out->model_us = h.model_us;
+    for (int l = 0; l < n_layers; ++l) {
+        out->tiles[l] = h.tiles[l];
+        out->split_k[l] = h.split[l];
+        out->reduce_mode[l] = h.reduce_mode[l];
+        out->ready_inc[l] = h.ready_inc[l];
+        out->units[l] = static_cast<int>(h.table[l].size());
+    }
+    return MLP_OK;
+}
+
+int mlp_pipe_plan_units(int M, int n_layers, const int* widths, const mlp_mode* mode, int num_sms, int layer, mlp_unit* out,
+                        int max_units, int* n_out) {
+    if (!out || !n_out || !widths || n_layers < 1 || n_layers > kMaxLayers || M < 1 || num_sms < 1 || layer < 0 ||
+        layer >= n_layers || max_units < 0)
+        return MLP_ERR_INVALID;
+    for (int l = 0; l <= n_layers; ++l)
+        if (widths[l] < 8 || widths[l] % 8 != 0) return MLP_ERR_INVALID;
+    mlp_mode m{};
+    if (mode) m = *mode;
+    else m.kind = MLP_CTA_PIPELINED;
+    int rc = validate_mode(m, M);
+    if (rc) return rc;
+    mlp_pipe h;
+    h.M = M;
+    h.L = n_layers;
+    for (int l = 0; l <= n_layers; ++l) h.widths[l] = widths[l];
+    h.mode = m;
+    h.num_sms = num_sms;
+    resolve(&h);
+    const std::vector<UnitDesc>& t = h.table[layer];
+    const int n = std::min<int>(max_units, static_cast<int>(t.size()));
+    for (int i = 0; i < n; ++i) {
+        out[i].tile = t[i].tile;
+        out[i].kind = t[i].kind;
+        out[i].k_slice = t[i].ks;
+        out[i].begin = t[i].a;
+        out[i].end = t[i].b;
+    }
+    *n_out = static_cast<int>(t.size());
+    return MLP_OK;
 }
 
 const char* mlp_status_string(int status) {

@@ -1,0 +1,118 @@
+"""Host logic of the ticket scheduler (step a1) checked WITHOUT a GPU: the unit tables
+that mlp_pipe_plan_units returns are what the persistent kernel walks ticket by ticket, so their invariants are
+the deadlock-freedom argument of DESIGN.md written as assertions."""
+import pytest
+
+from paper_2607_07862_b200 import binding as B
+from paper_2607_07862_b200 import inputs
+
+S, MB, P = B.MLP_SEQUENTIAL, B.MLP_MICROBATCH, B.MLP_CTA_PIPELINED
+
+SHAPES = [(c.M, tuple(c.widths)) for c in inputs.CONFIGS] + [
+    (1, (8, 8, 8)), (7, (72, 136, 8)), (300, (136, 264, 136)), (130, (264, 392, 200)), (16, (64, 128, 128, 128)),
+    (1024, (8192, 8192, 8192)),
+]
+MODES = [
+    dict(kind=P), dict(kind=S), dict(kind=MB, chunks=1), dict(kind=P, sm_split=0.5), dict(kind=P, split_k=4),
+    dict(kind=P, split_k=3, flags=B.MLP_FLAG_DEBUG_REVERSE), dict(kind=P, tile_n=256, tile_m=64), dict(kind=P, tile_n=128),
+    dict(kind=P, split_k_layer=[2, 9]), dict(kind=S, split_k=16),
+]
+
+
+def _check_tables(M, widths, plan, tables):
+    L = len(widths) - 1
+    rows = M
+    assert plan.tile_m % 16 == 0 and 16 <= plan.tile_m <= 256 and plan.tile_n in (128, 256)
+    assert plan.m_blks * plan.tile_m >= rows
+    assert plan.acc_stages * (plan.tile_n // 128) * plan.tile_m <= 512, "accumulator ring must fit the 512 TMEM columns"
+    assert plan.smem_bytes <= 227 * 1024
+    for l in range(L):
+        K, N = widths[l], widths[l + 1]
+        kb_total = -(-K // 64)
+        tiles = plan.m_blks * -(-N // plan.tile_n)
+        assert plan.tiles[l] == tiles
+        sp = plan.split_k[l]
+        table = tables[l]
+        assert len(table) == plan.units[l]
+        mma = [u for u in table if u[1] == 0]
+        red = [u for u in table if u[1] == 1]
+        # every (tile, K-slice) exactly once, and the slices of a tile tile [0, kb_total) without gap or overlap
+        assert len(mma) == tiles * sp
+        assert len({(t, ks) for t, _, ks, _, _ in mma}) == tiles * sp
+        per_tile = {}
+        for t, _, ks, a, b in mma:
+            assert 0 <= t < tiles and 0 <= ks < sp and a < b
+            per_tile.setdefault(t, []).append((a, b))
+        for t, spans in per_tile.items():
+            spans.sort()
+            assert spans[0][0] == 0 and spans[-1][1] == kb_total
+            assert all(spans[i][1] == spans[i + 1][0] for i in range(len(spans) - 1))
+        mode = plan.reduce_mode[l]
+        if sp == 1:
+            assert mode == 0 and not red and plan.ready_inc[l] == 1
+        elif mode == 1:
+            assert not red and plan.ready_inc[l] == 1
+        else:
+            assert mode == 2
+            # the reduce units of a tile partition its token columns, and every one of them holds a HIGHER ticket
+            # than all K-slices of its tile (a unit only ever waits on lower tickets: no deadlock)
+            pos_last_slice = {}
+            for i, u in enumerate(table):
+                if u[1] == 0:
+                    pos_last_slice[u[0]] = i
+            cols = {}
+            for i, u in enumerate(table):
+                if u[1] == 1:
+                    assert i > pos_last_slice[u[0]]
+                    assert u[3] % 16 == 0 and u[3] < u[4] <= plan.tile_m
+                    cols.setdefault(u[0], []).append((u[3], u[4]))
+            assert set(cols) == set(range(tiles))
+            for t, spans in cols.items():
+                spans.sort()
+                assert spans[0][0] == 0 and spans[-1][1] == plan.tile_m and len(spans) == plan.ready_inc[l]
+                assert all(spans[i][1] == spans[i + 1][0] for i in range(len(spans) - 1))
+
+
+@pytest.mark.parametrize("M,widths", SHAPES)
+@pytest.mark.parametrize("mode", MODES, ids=[str(i) for i in range(len(MODES))])
+def test_unit_tables_are_a_valid_schedule(M, widths, mode):
+    kw = dict(mode)
+    m = B.make_mode(**kw)
+    if kw.get("tile_m") and kw["tile_m"] * 2 > 512:
+        pytest.skip("shape not supported")
+    plan, tables = B.plan(M, widths, m, num_sms=148)
+    _check_tables(M, widths, plan, tables)
+    assert plan.model_us > 0
+
+
+def test_plan_depends_on_sm_count_and_is_deterministic():
+    cfg = inputs.CONFIGS[1]
+    a, ta = B.plan(cfg.M, cfg.widths, B.make_mode(P), num_sms=148)
+    b, tb = B.plan(cfg.M, cfg.widths, B.make_mode(P), num_sms=148)
+    assert ta == tb and list(a.split_k) == list(b.split_k)
+    c, tc = B.plan(cfg.M, cfg.widths, B.make_mode(P), num_sms=64)
+    assert c.grid == 64
+    _check_tables(cfg.M, cfg.widths, c, tc)
+
+
+def test_pipelined_plan_orders_consumer_slices_by_k():
+    """K-slice-major order of a many-slice consumer layer: its first tickets cover the lowest K range, i.e. depend on
+    the producer's EARLIEST tiles only (what lets the consumer start while the producer is still running)."""
+    cfg = inputs.CONFIGS[1]
+    plan, tables = B.plan(cfg.M, cfg.widths, B.make_mode(P))
+    if plan.split_k[1] > 4:
+        first = tables[1][: plan.tiles[1]]
+        assert all(u[2] == 0 and u[3] == 0 for u in first)
+
+
+def test_plan_rejects_bad_arguments():
+    import ctypes
+    lib = B.load()
+    w = (ctypes.c_int * 3)(64, 128, 128)
+    out = B.mlp_plan()
+    assert lib.mlp_pipe_plan(16, 2, w, None, 148, None) == B.MLP_ERR_INVALID
+    assert lib.mlp_pipe_plan(0, 2, w, None, 148, ctypes.byref(out)) == B.MLP_ERR_INVALID
+    assert lib.mlp_pipe_plan(16, 2, w, None, 0, ctypes.byref(out)) == B.MLP_ERR_INVALID
+    bad = (ctypes.c_int * 3)(64, 100, 128)
+    assert lib.mlp_pipe_plan(16, 2, bad, None, 148, ctypes.byref(out)) == B.MLP_ERR_INVALID
+    assert lib.mlp_pipe_plan(16, 2, w, None, 148, ctypes.byref(out)) == B.MLP_OK
