@@ -604,7 +604,9 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                         const uint32_t full = bar_full + 8 * stage;
                         mbar_arrive_expect_tx(full, w_tile_bytes);
                         const uint32_t dst = smem_base + stage * w_tile_bytes;
-                        if (hint) tma_load_2d_hint(dst, tm, kb * kTileK, u.n_blk * tile_n, full, pol);
+                        if (P.flags & 0x200u)  // EXPERIMENT: contiguous 16 KB tiles (timing only, wrong data)
+                            tma_load_2d_hint(dst, tm, 0, (u.n_blk * P.layer[u.layer].kb_total + kb) * tile_n, full, pol);
+                        else if (hint) tma_load_2d_hint(dst, tm, kb * kTileK, u.n_blk * tile_n, full, pol);
                         else tma_load_2d(dst, tm, kb * kTileK, u.n_blk * tile_n, full);
                         if (++stage == static_cast<uint32_t>(stages)) { stage = 0; phase ^= 1; }
                     }

@@ -164,7 +164,7 @@ constexpr double kSmBytesPerUs = 115e3;
 constexpr double kSmFlopsPerUs = 13.0e6;
 constexpr double kDramLatencyUs = 1.3;
 constexpr double kSmStoreBytesPerUs = 45e3;       // st.global of fp32 partials while the rings stream
-constexpr double kUnitOverheadUs = 0.15;
+constexpr double kUnitOverheadUs = 0.30;
 constexpr double kFenceUs = 0.10;
 constexpr double kPublishLatencyUs = 1.5;
 
@@ -194,6 +194,25 @@ struct Planner {
             if (rem - sz < lo) sz = rem;
             b.push_back(b.back() + sz);
             rem -= sz;
+        }
+        return b;
+    }
+    // n slices whose sizes fall linearly from r x to 1 x the last one (largest units first, so that the
+    // dynamic ticket ends the launch with small units and a short ragged tail), each at least `lo` K-blocks
+    std::vector<int> linear_taper(int l, int n, double r, int lo) const {
+        const int total = kb_total[l];
+        n = std::max(1, std::min(n, total / std::max(1, lo)));
+        std::vector<double> w(n);
+        double sum = 0.0;
+        for (int i = 0; i < n; ++i) sum += (w[i] = n > 1 ? r - (r - 1.0) * i / (n - 1) : 1.0);
+        std::vector<int> b{0};
+        double acc = 0.0;
+        for (int i = 0; i < n; ++i) {
+            acc += w[i] / sum * total;
+            int e = i == n - 1 ? total : static_cast<int>(acc + 0.5);
+            e = std::max(e, b.back() + lo);
+            e = std::min(e, total - (n - 1 - i) * lo);
+            b.push_back(e);
         }
         return b;
     }
@@ -442,6 +461,12 @@ void resolve(mlp_pipe* h) {
                         std::vector<int> t = pl.tapered(l, kb_floor, cap);
                         if (t.size() - 1 > 4 && t.size() - 1 <= 64) cand.push_back(t);
                     }
+                if (l == le - 1 && !pl.force_tile_major && !pl.producer_in_launch(l))
+                    for (int n : {6, 7, 8, 10, 12, 14, 16, 20, 24})
+                        for (double r : {2.0, 4.0, 6.0}) {
+                            std::vector<int> t = pl.linear_taper(l, n, r, std::max(4, kb_floor / 2));
+                            if (t.size() - 1 > 4) cand.push_back(t);
+                        }
                 std::vector<int> best = h->bounds[l];
                 pl.build_table(l, best, h->table[l], h->reduce_mode[l], h->ready_inc[l]);
                 double best_t = pl.makespan(lb, le);
@@ -458,6 +483,23 @@ void resolve(mlp_pipe* h) {
     if (pl.pipelined) refine(0, h->L);
     else
         for (int l = 0; l < h->L; ++l) refine(l, l + 1);
+    for (int l = 0; l < h->L; ++l) {  // experiments: MLP_PIPE_BOUNDS_<l>="0,24,..,<kb_total>" overrides the slices of layer l
+        char name[32];
+        snprintf(name, sizeof name, "MLP_PIPE_BOUNDS_%d", l);
+        const char* e = getenv(name);
+        if (!e) continue;
+        std::vector<int> b;
+        for (const char* q = e; *q;) {
+            b.push_back(atoi(q));
+            while (*q && *q != ',') ++q;
+            if (*q == ',') ++q;
+        }
+        bool ok = b.size() >= 2 && b.size() <= 256 && b.front() == 0 && b.back() == pl.kb_total[l];
+        for (size_t i = 1; ok && i < b.size(); ++i) ok = b[i] > b[i - 1];
+        if (!ok) continue;
+        h->bounds[l] = b;
+        pl.build_table(l, b, h->table[l], h->reduce_mode[l], h->ready_inc[l]);
+    }
     for (int l = 0; l < h->L; ++l) h->split[l] = static_cast<int>(h->bounds[l].size()) - 1;
     h->model_us = 0.0;
     if (pl.pipelined) h->model_us = pl.makespan(0, h->L);
@@ -686,7 +728,10 @@ int run_impl(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStre
     KernelParams P = h->base;
     if ((rc = lookup_tmap(h, h->cache_x, &h->cache_x_next, X, h->M, h->widths[0], h->tile_m, &P.tm_a[0]))) return rc;
     for (int l = 0; l < h->L; ++l)
-        if ((rc = lookup_tmap(h, h->cache_w[l], &h->cache_w_next[l], W[l], h->widths[l + 1], h->widths[l], kTileN * h->n_sub, &P.tm_w[l])))
+        if (h->mode.flags & 0x200u) {  // EXPERIMENT: view W as [N K / 64 x 64]: a box is 16 KB of contiguous memory
+            if ((rc = lookup_tmap(h, h->cache_w[l], &h->cache_w_next[l], W[l], h->widths[l + 1] * (h->widths[l] / 64), 64, kTileN * h->n_sub, &P.tm_w[l])))
+                return rc;
+        } else if ((rc = lookup_tmap(h, h->cache_w[l], &h->cache_w_next[l], W[l], h->widths[l + 1], h->widths[l], kTileN * h->n_sub, &P.tm_w[l])))
             return rc;
     P.layer[h->L - 1].out = static_cast<__nv_bfloat16*>(Y);
 
