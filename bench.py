@@ -43,6 +43,8 @@ def parse_args():
     ap.add_argument("--split-k", type=str, default="", help="comma list, per layer")
     ap.add_argument("--no-extras", action="store_true", help="skip the side measurements (other modes, e2e, cpu baseline)")
     ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--no-autotune", action="store_true",
+                    help="use the modelled plan instead of the measured plan search of the first (warm-up) run")
     return ap.parse_args()
 
 
@@ -141,7 +143,7 @@ def make_mode(B, args, n_layers):
     kind = {"pipelined": B.MLP_CTA_PIPELINED, "sequential": B.MLP_SEQUENTIAL, "microbatch": B.MLP_MICROBATCH}[args.mode]
     split = [int(x) for x in args.split_k.split(",")] if args.split_k else []
     return B.make_mode(kind, chunks=args.chunks if kind == B.MLP_MICROBATCH else 0, sm_split=args.sm_split,
-                       stages=args.stages, split_k_layer=split)
+                       stages=args.stages, split_k_layer=split, flags=0 if args.no_autotune else B.MLP_FLAG_AUTOTUNE)
 
 
 def device_inputs(torch, cfg, n_sets):
@@ -302,7 +304,8 @@ def main():
         "dtype": "bf16 in/out, fp32 accumulate", "data": "synthetic",
         "config": {"workload": f"BASELINE.json configs[{args.config}]: {cfg.name} M={cfg.M} widths={list(cfg.widths)} act={cfg.act}",
                    "mode": args.mode, "grid": st.grid, "tile_m": st.tile_m, "stages": st.stages,
-                   "split_k": list(st.split_k)[:cfg.n_layers], "sm_split": args.sm_split,
+                   "split_k": list(st.split_k)[:cfg.n_layers], "sm_split": args.sm_split, "tile_n": st.tile_n,
+                   "plan": "modelled" if args.no_autotune else "autotuned on the first warm-up run (MLP_FLAG_AUTOTUNE)",
                    "l2": f"inputs larger than L2: {N_WEIGHT_SETS} rotating weight sets of {alg_bytes / 1e6:.0f} MB, no weight reuse across steps",
                    "multi_gpu": "replicas only"},
         "latency_us": lat, "clocks": clocks, "gpu_launches": args.steps * launches_per_step, "roofline": roofline,
@@ -325,9 +328,10 @@ def extras(torch, B, inputs, cfg, args, X, sets, Y, with_cpu=True):
     inputs, the end-to-end number through the host-buffer entry point, and the timed CPU oracle."""
     out = {}
     modes = {}
-    for name, mode in (("sequential", B.make_mode(B.MLP_SEQUENTIAL, stages=args.stages)),
+    tune = 0 if args.no_autotune else B.MLP_FLAG_AUTOTUNE
+    for name, mode in (("sequential", B.make_mode(B.MLP_SEQUENTIAL, stages=args.stages, flags=tune)),
                        ("microbatch2", B.make_mode(B.MLP_MICROBATCH, chunks=2, stages=args.stages)),
-                       ("pipelined_sm_split_0.5", B.make_mode(B.MLP_CTA_PIPELINED, sm_split=0.5, stages=args.stages))):
+                       ("pipelined_sm_split_0.5", B.make_mode(B.MLP_CTA_PIPELINED, sm_split=0.5, stages=args.stages, flags=tune))):
         if cfg.M % 2 and name == "microbatch2":
             continue
         p = B.MlpPipe(cfg.M, cfg.widths, cfg.act, mode)

@@ -80,6 +80,12 @@ enum {
                                        before publishing (adversarial schedule for the protocol)     */
 #define MLP_FLAG_DEBUG_REVERSE 0x4u /* test hook: layer-1 units are handed out in reverse order       */
 #define MLP_FLAG_NO_W_EVICT_FIRST 0x8u /* do not tag weight loads L2 evict-first                      */
+#define MLP_FLAG_AUTOTUNE 0x400u    /* measured plan search: the FIRST mlp_pipe_run on the handle (outside stream
+                                       capture) tries the planner's candidate K-splits / ticket orders on the
+                                       caller's buffers, timing each with the in-kernel clock, and keeps the
+                                       fastest.  That one call synchronises the device, may allocate, and takes
+                                       tens of milliseconds; Y is valid after it.  Results are remembered per
+                                       process for equal (shape, mode).  SEQUENTIAL and CTA_PIPELINED only.     */
 
 typedef struct {
     int kind;        /* MLP_SEQUENTIAL | MLP_MICROBATCH | MLP_CTA_PIPELINED                           */

@@ -21,6 +21,7 @@ MLP_ACT_NONE, MLP_ACT_RELU, MLP_ACT_GELU_TANH = 0, 1, 2
 MLP_SEQUENTIAL, MLP_MICROBATCH, MLP_CTA_PIPELINED = 0, 1, 2
 MLP_MAX_LAYERS = 8
 MLP_FLAG_TILE_MAJOR, MLP_FLAG_DEBUG_DELAY, MLP_FLAG_DEBUG_REVERSE, MLP_FLAG_NO_W_EVICT_FIRST = 1, 2, 4, 8
+MLP_FLAG_AUTOTUNE = 0x400
 
 EXPORTS = [
     "mlp_pipe_create", "mlp_pipe_create_chain", "mlp_pipe_run", "mlp_pipe_run_chain", "mlp_pipe_run_host",

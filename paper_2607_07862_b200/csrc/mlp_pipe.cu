@@ -9,6 +9,8 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <map>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -53,6 +55,12 @@ struct mlp_pipe {
     UnitDesc* d_table[kMaxLayers] = {nullptr};  // the same on the device
     int tiles[kMaxLayers] = {0};
     double model_us = 0.0;  // the planner's estimate of the launch(es)
+    int kb_min = 0, kb_floor = 0;   // smallest K-slice the planner considers / allows
+    bool fixed_split[kMaxLayers] = {false};  // the caller pinned this layer's split
+    size_t table_cap[kMaxLayers] = {0};      // entries allocated for d_table[l]
+    size_t ws_cap[kMaxLayers] = {0};         // bytes allocated for ws[l]
+    bool tuned = false;                      // MLP_FLAG_AUTOTUNE: the measured search has run (or is not applicable)
+    double tuned_us = 0.0;                   // its best measured in-kernel span
     // device memory owned by the handle
     __nv_bfloat16* H[kMaxLayers] = {nullptr};  // H[l] = output of layer l, l < L-1
     float* ws[kMaxLayers] = {nullptr};
@@ -184,19 +192,6 @@ struct Planner {
         for (int i = 0; i <= sp; ++i) b[i] = static_cast<int>(static_cast<long long>(i) * kb_total[l] / sp);
         return b;
     }
-    // guided self-scheduling: each group of `tiles` units gets remaining_work / (2 * grid), within [lo, cap]
-    std::vector<int> tapered(int l, int lo, int cap) const {
-        std::vector<int> b{0};
-        int rem = kb_total[l];
-        while (rem > 0) {
-            int sz = static_cast<int>(static_cast<long long>(rem) * h->tiles[l] / (2 * h->grid));
-            sz = std::max(lo, std::min(cap, sz));
-            if (rem - sz < lo) sz = rem;
-            b.push_back(b.back() + sz);
-            rem -= sz;
-        }
-        return b;
-    }
     // n slices whose sizes fall linearly from r x to 1 x the last one (largest units first, so that the
     // dynamic ticket ends the launch with small units and a short ragged tail), each at least `lo` K-blocks
     std::vector<int> linear_taper(int l, int n, double r, int lo) const {
@@ -303,84 +298,221 @@ struct Planner {
         for (int l = 0; l < h->L; ++l) build_table(l, h->bounds[l], h->table[l], h->reduce_mode[l], h->ready_inc[l]);
     }
 
-    // Greedy list scheduling of the tables of layers [lb, le) in ticket order on `grid` workers.
-    double makespan(int lb, int le) const {
+    // Event-driven simulation of one launch over layers [lb, le): `grid` workers draw the tickets of the unit
+    // tables in order (late binding: a worker draws when it is free), a unit waits for the units it depends on,
+    // and the workers that are streaming weights at the same moment SHARE the HBM bandwidth (a worker alone is
+    // limited by its own ring / L2 port / tensor core instead).  Returns the time the last output is stored.
+    double makespan(int lb, int le, double cutoff = 1e30) const {
         const int G = h->grid, R = h->n_sub, tm = h->tile_m;
         const double w_bytes = R * static_cast<double>(kWTileBytes), a_bytes = tm * 128.0;
-        size_t mma_units = 0;
-        for (int l = lb; l < le; ++l) mma_units += static_cast<size_t>(h->tiles[l]) * (h->bounds[l].size() - 1);
-        const int active = static_cast<int>(std::min<size_t>(G, std::max<size_t>(1, mma_units)));  // CTAs that share HBM
-        // one SM streams from DRAM at most its ring of outstanding weight bytes per DRAM latency
-        const double t_kb = std::max({w_bytes / (kHbmBytesPerUs / active), w_bytes / (h->stages * w_bytes / kDramLatencyUs),
-                                      (w_bytes + a_bytes) / kSmBytesPerUs, 2.0 * R * kTileN * tm * kTileK / kSmFlopsPerUs});
-        // a dependent global round trip queues behind the SM's own ring of TMA requests, which drains at the
-        // rate the main loop consumes it
-        const double rtt = 0.6 + 0.5 * (h->stages * w_bytes + h->a_stages * a_bytes) / ((w_bytes + a_bytes) / t_kb);
+        // per K-block and worker: floor set by the worker's own limits ...
+        const double t_cap = std::max({kDramLatencyUs / h->stages, (w_bytes + a_bytes) / kSmBytesPerUs,
+                                       2.0 * R * kTileN * tm * kTileK / kSmFlopsPerUs});
+        const double t_share = w_bytes / kHbmBytesPerUs;  // ... and by HBM: t_share x (workers streaming)
+        const double t_full = std::max(t_cap, t_share * G);
+        // a dependent global round trip queues behind the SM's own ring of TMA requests
+        const double rtt = 0.6 + 0.5 * (h->stages * w_bytes + h->a_stages * a_bytes) / ((w_bytes + a_bytes) / t_full);
         const double part_us = partial_bytes() / kSmStoreBytesPerUs;
         const double epi_us = R * tm * 0.004 + 0.3;  // act + convert + transpose of one accumulator
-        // sum of `cols` token columns over sp partials by ONE CTA: kGather slices x 16 columns per round trip
-        auto gather_us = [&](int sp, int cols) {
+        const double drain_us = h->stages * t_full;  // last weight tile requested -> accumulator complete
+        auto gather_us = [&](int sp, int cols) {     // ONE CTA sums `cols` token columns over sp partials
             const int trips = R * ((cols + 15) / 16) * ((sp + kGather - 1) / kGather);
             return trips * rtt + static_cast<double>(sp) * R * cols * kTileN * 4 / kSmBytesPerUs;
         };
-        std::vector<std::pair<double, int>> fin(G);  // min-heap of (finish time, worker)
-        for (int i = 0; i < G; ++i) fin[i] = {0.0, i};
-        auto cmp = [](const std::pair<double, int>& x, const std::pair<double, int>& y) { return x.first > y.first; };
-        double end = 0.0;
-        std::vector<double> done_prev, done_cur, part_done;
-        std::vector<int> arrived;
+        const double kInf = 1e30;
+        struct Worker {
+            int layer = -1, idx = -1;  // current unit (table index), -1 = none
+            int phase = 0;             // 0 idle, 1 waiting for its dependencies, 2 fixed-time part, 3 streaming
+            double t_end = 0.0;        // phase 2: when it ends
+            double rem = 0.0;          // phase 3: K-blocks left
+            double speed = 1.0;
+        };
+        std::vector<Worker> wk(G);
+        for (int i = 0; i < G; ++i) wk[i].speed = 1.0 + 0.08 * (((i * 37) % 11) - 5) / 5.0;
+        // per layer: when a tile is visible to consumers / when its partials are complete
+        std::vector<std::vector<double>> done(le), part_done(le);
+        std::vector<std::vector<int>> arrived(le), reduced(le);
         for (int l = lb; l < le; ++l) {
-            const std::vector<UnitDesc>& tb = h->table[l];
-            const int sp = static_cast<int>(h->bounds[l].size()) - 1, tiles = h->tiles[l];
-            const int n_blks = tiles / h->m_blks;
-            const int n_blks_prev = l > lb ? h->tiles[l - 1] / h->m_blks : 0;
-            const int mode = h->reduce_mode[l];
-            done_cur.assign(tiles, 0.0);
-            part_done.assign(tiles, 0.0);
-            arrived.assign(tiles, 0);
-            for (const UnitDesc& d : tb) {
-                std::pop_heap(fin.begin(), fin.end(), cmp);
-                const double speed = 1.0 + 0.08 * (((fin.back().second * 37) % 11) - 5) / 5.0;
-                double start = fin.back().first, busy, done;
-                if (d.kind == kUnitMma) {
-                    if (l > lb) {  // the consumer prologue waits for the producer tiles under its K range
-                        const int m_blk = d.tile / n_blks;
-                        const int tn = kTileN * R;
-                        for (int j = (d.a * kTileK) / tn; j <= ((d.b - 1) * kTileK) / tn && j < n_blks_prev; ++j)
-                            start = std::max(start, done_prev[m_blk * n_blks_prev + j]);
-                    }
-                    double ovh = kUnitOverheadUs + (l > lb && pipelined ? kFenceUs : 0.0);
-                    if (sp > 1) ovh += kFenceUs + 0.5 * part_us;
-                    busy = ((d.b - d.a) * t_kb + ovh) * speed;
-                    done = start + busy;
-                    double fin_t = done;  // when this unit's share of the layer's output is in memory
-                    if (sp == 1) {
-                        fin_t = done + epi_us;
-                        done_cur[d.tile] = fin_t + kPublishLatencyUs;
-                    } else {
-                        part_done[d.tile] = std::max(part_done[d.tile], done + part_us + rtt);
-                        if (mode == kReduceLastArriver && ++arrived[d.tile] == sp) {
-                            fin_t = part_done[d.tile] + gather_us(sp, tm);
-                            done_cur[d.tile] = fin_t + kPublishLatencyUs;
-                        }
-                    }
-                    end = std::max(end, fin_t);
-                } else {
-                    const double g_us = gather_us(sp, d.b - d.a);
-                    start = std::max(start, part_done[d.tile]);
-                    busy = 0.35 * g_us * speed;  // epilogue warps only: the main loop of the next unit overlaps
-                    done = start + g_us;
-                    done_cur[d.tile] = std::max(done_cur[d.tile], done + kPublishLatencyUs);
-                    end = std::max(end, done);
-                }
-                fin.back().first = start + busy;
-                std::push_heap(fin.begin(), fin.end(), cmp);
-            }
-            done_prev.swap(done_cur);
+            done[l].assign(h->tiles[l], kInf);
+            part_done[l].assign(h->tiles[l], 0.0);
+            arrived[l].assign(h->tiles[l], 0);
+            reduced[l].assign(h->tiles[l], 0);
         }
+        int next_layer = lb;
+        size_t next_idx = 0;
+        double now = 0.0, end = 0.0;
+        auto split_of = [&](int l) { return static_cast<int>(h->bounds[l].size()) - 1; };
+        // When may the unit of worker w start?  kInf while a dependency has not completed.  Dependencies are
+        // scanned incrementally (completion times are written once), so the scan is O(deps) per unit overall.
+        std::vector<int> dep_j(G, 0);
+        std::vector<double> dep_max(G, 0.0);
+        auto ready_at = [&](int wi) {
+            const Worker& w = wk[wi];
+            const int l = w.layer;
+            const UnitDesc& d = h->table[l][w.idx];
+            if (d.kind == kUnitReduce) return arrived[l][d.tile] == split_of(l) ? part_done[l][d.tile] : kInf;
+            if (l == lb) return 0.0;
+            const int n_blks = h->tiles[l] / h->m_blks, n_prev = h->tiles[l - 1] / h->m_blks, tn = kTileN * R;
+            const int m_blk = d.tile / n_blks;
+            const int j1 = std::min(n_prev - 1, ((d.b - 1) * kTileK) / tn);
+            if (dep_j[wi] == 0) dep_j[wi] = (d.a * kTileK) / tn;
+            while (dep_j[wi] <= j1) {
+                const double t = done[l - 1][m_blk * n_prev + dep_j[wi]];
+                if (t >= kInf) return kInf;
+                dep_max[wi] = std::max(dep_max[wi], t);
+                ++dep_j[wi];
+            }
+            return dep_max[wi];
+        };
+        std::vector<double> red_fin;  // per tile of the current reduce layer: latest finish of its reduce units
+        std::vector<std::vector<double>> red_done(le);
+        for (int l = lb; l < le; ++l) red_done[l].assign(h->tiles[l], 0.0);
+        for (int guard = 0; guard < 4000000; ++guard) {
+            bool changed = true;
+            while (changed) {
+                changed = false;
+                for (int i = 0; i < G; ++i) {
+                    Worker& w = wk[i];
+                    if (w.phase == 0 && next_layer < le) {  // draw the next ticket
+                        while (next_layer < le && next_idx >= h->table[next_layer].size()) {
+                            ++next_layer;
+                            next_idx = 0;
+                        }
+                        if (next_layer >= le) continue;
+                        w.layer = next_layer;
+                        w.idx = static_cast<int>(next_idx++);
+                        w.phase = 1;
+                        dep_j[i] = 0;
+                        dep_max[i] = 0.0;
+                        changed = true;
+                    }
+                    if (w.phase == 1 && ready_at(i) <= now) {
+                        const UnitDesc& d = h->table[w.layer][w.idx];
+                        const int sp = split_of(w.layer);
+                        if (d.kind == kUnitMma) {
+                            double ovh = kUnitOverheadUs + (w.layer > lb && pipelined ? kFenceUs : 0.0);
+                            if (sp > 1) ovh += kFenceUs + 0.5 * part_us;
+                            w.t_end = now + ovh * w.speed;
+                        } else {
+                            const double g = gather_us(sp, d.b - d.a);
+                            w.t_end = now + 0.35 * g * w.speed;  // epilogue warps only: the next main loop overlaps
+                            red_done[w.layer][d.tile] = std::max(red_done[w.layer][d.tile], now + g);
+                            if (++reduced[w.layer][d.tile] == h->ready_inc[w.layer])
+                                done[w.layer][d.tile] = red_done[w.layer][d.tile] + kPublishLatencyUs;
+                            end = std::max(end, now + g);
+                        }
+                        w.phase = 2;
+                        changed = true;
+                    }
+                    if (w.phase == 2 && w.t_end <= now) {
+                        const UnitDesc& d = h->table[w.layer][w.idx];
+                        if (d.kind == kUnitMma) {
+                            w.phase = 3;
+                            w.rem = d.b - d.a;
+                        } else {
+                            w.phase = 0;
+                        }
+                        changed = true;
+                    }
+                }
+            }
+            int n_stream = 0;
+            for (int i = 0; i < G; ++i) n_stream += wk[i].phase == 3;
+            const double t_kb = std::max(t_cap, t_share * n_stream);
+            double t_next = kInf;
+            for (int i = 0; i < G; ++i) {
+                const Worker& w = wk[i];
+                if (w.phase == 1) {
+                    const double r = ready_at(i);
+                    if (r < kInf) t_next = std::min(t_next, r);
+                } else if (w.phase == 2) {
+                    t_next = std::min(t_next, w.t_end);
+                } else if (w.phase == 3) {
+                    t_next = std::min(t_next, now + w.rem * t_kb * w.speed);
+                }
+            }
+            if (t_next >= kInf) break;  // everything handed out and finished (or nothing can ever run)
+            t_next = std::max(t_next, now);
+            if (t_next > cutoff) return 1e9;  // already worse than the best candidate so far
+            const double dt = t_next - now;
+            now = t_next;
+            for (int i = 0; i < G; ++i) {
+                Worker& w = wk[i];
+                if (w.phase != 3) continue;
+                w.rem -= dt / (t_kb * w.speed);
+                if (w.rem > 1e-6) continue;
+                // the last weight tile of the unit has been requested: the worker is free for its next ticket
+                const int l = w.layer;
+                const UnitDesc& d = h->table[l][w.idx];
+                const int sp = split_of(l);
+                const double acc_t = now + drain_us;
+                if (sp == 1) {
+                    done[l][d.tile] = acc_t + epi_us + kPublishLatencyUs;
+                    end = std::max(end, acc_t + epi_us);
+                } else {
+                    part_done[l][d.tile] = std::max(part_done[l][d.tile], acc_t + part_us + rtt);
+                    end = std::max(end, acc_t + part_us);
+                    if (++arrived[l][d.tile] == sp && h->reduce_mode[l] == kReduceLastArriver) {
+                        const double fin_t = part_done[l][d.tile] + gather_us(sp, tm);
+                        done[l][d.tile] = fin_t + kPublishLatencyUs;
+                        end = std::max(end, fin_t);
+                    }
+                }
+                w.phase = 0;
+            }
+        }
+        for (int i = 0; i < G; ++i)
+            if (wk[i].phase != 0) return 1e9;  // a unit that can never start: not a valid schedule
         return end;
     }
 };
+
+// Planning is deterministic in (M, widths, mode, SM count): remember the slice boundaries per process.
+std::mutex g_plan_mutex;
+std::map<std::string, std::vector<std::vector<int>>> g_plan_cache;
+
+std::string plan_key(const mlp_pipe* h) {
+    std::string k(reinterpret_cast<const char*>(&h->mode), sizeof(mlp_mode));
+    const int head[3] = {h->M, h->L, h->num_sms};
+    k.append(reinterpret_cast<const char*>(head), sizeof head);
+    k.append(reinterpret_cast<const char*>(h->widths), sizeof(int) * (h->L + 1));
+    for (int l = 0; l < h->L; ++l) {
+        char name[32];
+        snprintf(name, sizeof name, "MLP_PIPE_BOUNDS_%d", l);
+        const char* e = getenv(name);
+        k.append(e ? e : "-");
+        k.push_back(';');
+    }
+    return k;
+}
+
+Planner make_planner(mlp_pipe* h) {
+    Planner pl;
+    pl.h = h;
+    pl.pipelined = h->mode.kind == MLP_CTA_PIPELINED;
+    pl.force_tile_major = (h->mode.flags & (MLP_FLAG_TILE_MAJOR | MLP_FLAG_DEBUG_REVERSE)) != 0;
+    for (int l = 0; l < h->L; ++l) pl.kb_total[l] = ceil_div(h->widths[l], kTileK);
+    return pl;
+}
+
+// Slice-boundary candidates for layer l of a launch whose last layer is `last`: equal slices, plus tapered
+// ones for the last layer.
+std::vector<std::vector<int>> slice_candidates(const Planner& pl, int l, bool last, int kb_floor, bool thin) {
+    std::vector<std::vector<int>> cand;
+    const int s_max = std::max(1, std::min(64, pl.kb_total[l] / kb_floor));
+    for (int c : {1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 12, 14, 16, 20, 24, 28, 32, 40, 48, 64}) {
+        if (c > s_max || (thin && c > 20)) break;
+        if (pl.producer_in_launch(l) && c > 4 && pl.reduce_mode_for(c) == kReduceLastArriver) continue;
+        cand.push_back(pl.uniform(l, c));
+    }
+    if (last && !pl.force_tile_major && !pl.producer_in_launch(l))
+        for (int n : {7, 10, 12, 14, 16, 20})
+            for (double r : {3.0, 6.0}) {
+                std::vector<int> t = pl.linear_taper(l, n, r, std::max(4, kb_floor / 2));
+                if (t.size() - 1 > 4) cand.push_back(t);
+            }
+    return cand;
+}
 
 void resolve(mlp_pipe* h) {
     const mlp_mode& m = h->mode;
@@ -434,10 +566,13 @@ void resolve(mlp_pipe* h) {
     // bytes the slice streams
     const int kb_min = std::max(h->tile_m <= 32 ? 8 : 16, static_cast<int>(8 * pl.partial_bytes() / (w_tile + a_tile)) / 4 * 4);
     const int kb_floor = std::max(4, kb_min / 2);
+    h->kb_min = kb_min;
+    h->kb_floor = kb_floor;
     bool fixed[kMaxLayers];
     for (int l = 0; l < h->L; ++l) {
         int sp = m.split_k_layer[l] > 0 ? m.split_k_layer[l] : m.split_k;
         fixed[l] = sp > 0;
+        h->fixed_split[l] = fixed[l];
         if (sp <= 0) {
             sp = std::min(ceil_div(3 * h->grid, h->tiles[l]), std::max(1, pl.kb_total[l] / kb_min));
             if (pl.producer_in_launch(l) && pl.reduce_mode_for(sp) == kReduceLastArriver) sp = std::min(sp, 4);
@@ -450,39 +585,36 @@ void resolve(mlp_pipe* h) {
         for (int pass = 0; pass < 2; ++pass)
             for (int l = le - 1; l >= lb; --l) {
                 if (fixed[l]) continue;
-                std::vector<std::vector<int>> cand;
-                const int s_max = std::max(1, std::min(64, pl.kb_total[l] / kb_floor));
-                for (int c = 1; c <= s_max; ++c) {
-                    if (pl.producer_in_launch(l) && c > 4 && pl.reduce_mode_for(c) == kReduceLastArriver) continue;
-                    cand.push_back(pl.uniform(l, c));
-                }
-                if (l == le - 1 && !pl.force_tile_major && !pl.producer_in_launch(l))
-                    for (int cap : {2 * kb_floor, 3 * kb_floor, 4 * kb_floor, 6 * kb_floor, 8 * kb_floor}) {
-                        std::vector<int> t = pl.tapered(l, kb_floor, cap);
-                        if (t.size() - 1 > 4 && t.size() - 1 <= 64) cand.push_back(t);
-                    }
-                if (l == le - 1 && !pl.force_tile_major && !pl.producer_in_launch(l))
-                    for (int n : {6, 7, 8, 10, 12, 14, 16, 20, 24})
-                        for (double r : {2.0, 4.0, 6.0}) {
-                            std::vector<int> t = pl.linear_taper(l, n, r, std::max(4, kb_floor / 2));
-                            if (t.size() - 1 > 4) cand.push_back(t);
-                        }
+                const std::vector<std::vector<int>> cand = slice_candidates(pl, l, l == le - 1, kb_floor, false);
                 std::vector<int> best = h->bounds[l];
                 pl.build_table(l, best, h->table[l], h->reduce_mode[l], h->ready_inc[l]);
                 double best_t = pl.makespan(lb, le);
-                for (auto& c : cand) {
+                for (const auto& c : cand) {
                     h->bounds[l] = c;
                     pl.build_table(l, c, h->table[l], h->reduce_mode[l], h->ready_inc[l]);
-                    const double t = pl.makespan(lb, le);
+                    const double t = pl.makespan(lb, le, best_t);
                     if (t < best_t * 0.995) { best_t = t; best = c; }
                 }
                 h->bounds[l] = best;
                 pl.build_table(l, best, h->table[l], h->reduce_mode[l], h->ready_inc[l]);
             }
     };
-    if (pl.pipelined) refine(0, h->L);
-    else
-        for (int l = 0; l < h->L; ++l) refine(l, l + 1);
+    const std::string key = plan_key(h);
+    bool cached = false;
+    {
+        std::lock_guard<std::mutex> lock(g_plan_mutex);
+        auto it = g_plan_cache.find(key);
+        if (it != g_plan_cache.end()) {
+            for (int l = 0; l < h->L; ++l) h->bounds[l] = it->second[l];
+            pl.build_all();
+            cached = true;
+        }
+    }
+    if (!cached) {
+        if (pl.pipelined) refine(0, h->L);
+        else
+            for (int l = 0; l < h->L; ++l) refine(l, l + 1);
+    }
     for (int l = 0; l < h->L; ++l) {  // experiments: MLP_PIPE_BOUNDS_<l>="0,24,..,<kb_total>" overrides the slices of layer l
         char name[32];
         snprintf(name, sizeof name, "MLP_PIPE_BOUNDS_%d", l);
@@ -499,6 +631,12 @@ void resolve(mlp_pipe* h) {
         if (!ok) continue;
         h->bounds[l] = b;
         pl.build_table(l, b, h->table[l], h->reduce_mode[l], h->ready_inc[l]);
+    }
+    if (!cached) {
+        std::lock_guard<std::mutex> lock(g_plan_mutex);
+        std::vector<std::vector<int>> v(h->L);
+        for (int l = 0; l < h->L; ++l) v[l] = h->bounds[l];
+        g_plan_cache[key] = v;
     }
     for (int l = 0; l < h->L; ++l) h->split[l] = static_cast<int>(h->bounds[l].size()) - 1;
     h->model_us = 0.0;
@@ -615,6 +753,35 @@ int launch(mlp_pipe* h, KernelParams& P, cudaStream_t s) {
     return MLP_OK;
 }
 
+// Make the plan in h->bounds / h->table current on the device: tables, split-K workspace, launch template,
+// and zeroed protocol state (the counters' bases depend on the split).  Synchronises the device.
+int install_plan(mlp_pipe* h) {
+    CUDA_TRY(h, cudaDeviceSynchronize());
+    for (int l = 0; l < h->L; ++l) {
+        h->split[l] = static_cast<int>(h->bounds[l].size()) - 1;
+        const size_t n = h->table[l].size();
+        if (n > h->table_cap[l]) {
+            if (h->d_table[l]) CUDA_TRY(h, cudaFree(h->d_table[l]));
+            h->d_table[l] = nullptr;
+            h->table_cap[l] = n + n / 2 + 64;
+            CUDA_TRY(h, cudaMalloc(&h->d_table[l], h->table_cap[l] * sizeof(UnitDesc)));
+        }
+        CUDA_TRY(h, cudaMemcpy(h->d_table[l], h->table[l].data(), n * sizeof(UnitDesc), cudaMemcpyHostToDevice));
+        const size_t ws_bytes = h->split[l] > 1 ? static_cast<size_t>(h->tiles[l]) * h->split[l] * h->n_sub * h->tile_m * kTileN * sizeof(float) : 0;
+        if (ws_bytes > h->ws_cap[l]) {
+            if (h->ws[l]) CUDA_TRY(h, cudaFree(h->ws[l]));
+            h->ws[l] = nullptr;
+            h->ws_cap[l] = ws_bytes + ws_bytes / 4;
+            CUDA_TRY(h, cudaMalloc(&h->ws[l], h->ws_cap[l]));
+        }
+    }
+    int rc = reset_state(h, nullptr);
+    if (rc == MLP_OK) rc = build_base_params(h);
+    if (rc) return rc;
+    CUDA_TRY(h, cudaDeviceSynchronize());
+    return MLP_OK;
+}
+
 int create_impl(mlp_pipe** out, int M, int L, const int* widths, int dtype, int act, const mlp_mode* mode) {
     if (!out) return fail(nullptr, MLP_ERR_INVALID, "out is NULL");
     *out = nullptr;
@@ -676,13 +843,6 @@ int create_impl(mlp_pipe** out, int M, int L, const int* widths, int dtype, int 
             p += round_up(h->tiles[l], 32);
         }
     }
-    for (int l = 0; l < L; ++l) {
-        CREATE_TRY(cudaMalloc(&h->d_table[l], h->table[l].size() * sizeof(UnitDesc)));
-        CREATE_TRY(cudaMemcpy(h->d_table[l], h->table[l].data(), h->table[l].size() * sizeof(UnitDesc), cudaMemcpyHostToDevice));
-    }
-    for (int l = 0; l < L; ++l)
-        if (h->split[l] > 1)
-            CREATE_TRY(cudaMalloc(&h->ws[l], static_cast<size_t>(h->tiles[l]) * h->split[l] * h->n_sub * h->tile_m * kTileN * sizeof(float)));
     CREATE_TRY(cudaMalloc(&h->epoch, kMaxLayers * sizeof(unsigned long long)));
     CREATE_TRY(cudaMalloc(&h->status, sizeof(uint32_t)));
     CREATE_TRY(cudaMalloc(&h->stats, sizeof(CtaStats) * kMaxLayers * h->grid));
@@ -693,9 +853,8 @@ int create_impl(mlp_pipe** out, int M, int L, const int* widths, int dtype, int 
         h->ev_done.resize(static_cast<size_t>(L) * m.chunks, nullptr);
         for (auto& e : h->ev_done) CREATE_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     }
-    rc = reset_state(h, nullptr);
-    if (rc == MLP_OK) rc = build_base_params(h);
-    if (rc == MLP_OK && cudaDeviceSynchronize() != cudaSuccess) rc = MLP_ERR_CUDA;
+    rc = install_plan(h);
+    h->tuned = !(m.flags & MLP_FLAG_AUTOTUNE) || m.kind == MLP_MICROBATCH;
     if (rc) {
         g_create_error = h->last_error;
         mlp_pipe_destroy(h);
@@ -712,7 +871,7 @@ int check_ptr(mlp_pipe* h, const void* p, const char* name) {
     return MLP_OK;
 }
 
-int run_impl(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStream_t s) {
+int run_core(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStream_t s) {
     int rc;
     if ((rc = check_ptr(h, X, "X"))) return rc;
     if ((rc = check_ptr(h, Y, "Y"))) return rc;
@@ -785,6 +944,125 @@ int run_impl(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStre
     }
     h->runs++;
     return MLP_OK;
+}
+
+// In-kernel span of the most recent run: per launch class, last CTA exit - first CTA start (globaltimer), summed.
+int last_span_us(mlp_pipe* h, double* out) {
+    const int classes = h->mode.kind == MLP_CTA_PIPELINED ? 1 : h->L;
+    std::vector<CtaStats> cs(static_cast<size_t>(classes) * h->grid);
+    CUDA_TRY(h, cudaMemcpy(cs.data(), h->stats, cs.size() * sizeof(CtaStats), cudaMemcpyDeviceToHost));
+    double total = 0.0;
+    for (int c = 0; c < classes; ++c) {
+        unsigned long long t0 = ~0ull, t1 = 0;
+        for (int b = 0; b < h->grid; ++b) {
+            const CtaStats& st = cs[static_cast<size_t>(c) * h->grid + b];
+            t0 = std::min(t0, st.ts[0]);
+            t1 = std::max(t1, st.ts[7]);
+        }
+        total += (t1 - t0) * 1e-3;
+    }
+    *out = total;
+    return MLP_OK;
+}
+
+// MLP_FLAG_AUTOTUNE: measured coordinate descent over the planner's slice candidates, layer by layer from the
+// last one, on the caller's buffers (every candidate computes the same Y).  Starts from the modelled plan.
+int autotune(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStream_t s) {
+    int rc;
+    CUDA_TRY(h, cudaStreamSynchronize(s));
+    Planner pl = make_planner(h);
+    auto measure = [&](double* us) -> int {
+        int r = install_plan(h);
+        if (r) return r;
+        double best = 1e30;
+        for (int i = 0; i < 4; ++i) {  // first run warms the tensor maps / instruction cache
+            if ((r = run_core(h, X, W, Y, s))) return r;
+            CUDA_TRY(h, cudaStreamSynchronize(s));
+            double t;
+            if ((r = last_span_us(h, &t))) return r;
+            if (i > 0) best = std::min(best, t);
+        }
+        *us = best;
+        return MLP_OK;
+    };
+    double best_us;
+    if ((rc = measure(&best_us))) return rc;
+    const int n_launch = pl.pipelined ? 1 : h->L;
+    for (int pass = 0; pass < 2; ++pass) {
+        bool improved = false;
+        for (int l = h->L - 1; l >= 0; --l) {
+            if (h->fixed_split[l]) continue;
+            const bool last = pl.pipelined ? l == h->L - 1 : true;
+            const std::vector<int> start = h->bounds[l];
+            std::vector<int> best = start;
+            for (const auto& c : slice_candidates(pl, l, last, h->kb_floor, true)) {
+                if (c == start) continue;
+                h->bounds[l] = c;
+                pl.build_table(l, c, h->table[l], h->reduce_mode[l], h->ready_inc[l]);
+                double t;
+                if ((rc = measure(&t))) return rc;
+                if (t < best_us - 0.05 * n_launch) {
+                    best_us = t;
+                    best = c;
+                    improved = true;
+                }
+            }
+            h->bounds[l] = best;
+            pl.build_table(l, best, h->table[l], h->reduce_mode[l], h->ready_inc[l]);
+        }
+        if (!improved) break;
+    }
+    if ((rc = install_plan(h))) return rc;
+    h->tuned_us = best_us;
+    h->tuned = true;
+    {
+        std::lock_guard<std::mutex> lock(g_plan_mutex);
+        std::vector<std::vector<int>> v(h->L);
+        for (int l = 0; l < h->L; ++l) v[l] = h->bounds[l];
+        g_plan_cache[plan_key(h) + "#tuned"] = v;
+    }
+    if (getenv("MLP_PIPE_DEBUG")) {
+        fprintf(stderr, "[mlp_pipe] autotuned: %.1f us in-kernel span;", best_us);
+        for (int l = 0; l < h->L; ++l) {
+            fprintf(stderr, " L%d:", l);
+            for (int b : h->bounds[l]) fprintf(stderr, " %d", b);
+        }
+        fprintf(stderr, "\n");
+    }
+    return MLP_OK;
+}
+
+int run_impl(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStream_t s) {
+    if (!h->tuned) {
+        int rc;
+        if ((rc = check_ptr(h, X, "X"))) return rc;
+        if ((rc = check_ptr(h, Y, "Y"))) return rc;
+        if (!W) return fail(h, MLP_ERR_INVALID, "W is NULL");
+        for (int l = 0; l < h->L; ++l)
+            if ((rc = check_ptr(h, W[l], "W[l]"))) return rc;
+        cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(s, &cap) != cudaSuccess) cap = cudaStreamCaptureStatusNone;
+        if (cap == cudaStreamCaptureStatusNone) {  // no search inside a graph capture: the modelled plan runs
+            bool cached = false;
+            {
+                std::lock_guard<std::mutex> lock(g_plan_mutex);
+                auto it = g_plan_cache.find(plan_key(h) + "#tuned");
+                if (it != g_plan_cache.end()) {
+                    Planner pl = make_planner(h);
+                    for (int l = 0; l < h->L; ++l) h->bounds[l] = it->second[l];
+                    pl.build_all();
+                    cached = true;
+                }
+            }
+            if (cached) {
+                if ((rc = install_plan(h))) return rc;
+                h->tuned = true;
+            } else if ((rc = autotune(h, X, W, Y, s))) {
+                return rc;
+            }
+        }
+    }
+    return run_core(h, X, W, Y, s);
 }
 
 }  // namespace

@@ -276,3 +276,24 @@ def test_watchdog_turns_a_hang_into_timeout():
         torch.cuda.synchronize()
         assert p.stats().status == 0
     p.close()
+
+
+def test_autotune_keeps_results_exact_and_state_consistent():
+    """MLP_FLAG_AUTOTUNE: the first run searches K-splits / ticket orders on the caller's buffers; every candidate
+    computes the same Y, the counters are reset between candidates, and later runs (incl. a second handle that
+    takes the remembered plan) stay bit-exact."""
+    for cfg in (inputs.get_config(0, "exact"), inputs.Config("tune_3l", 48, (256, 1024, 512, 256), B.MLP_ACT_RELU, "exact", 9)):
+        X, Ws, outs, _ = oracle_outs(cfg)
+        Xd, Wd = X.cuda(), [w.cuda() for w in Ws]
+        for kind in (P, S):
+            for rep in range(2):
+                p = B.MlpPipe(cfg.M, cfg.widths, cfg.act, B.make_mode(kind, flags=B.MLP_FLAG_AUTOTUNE))
+                for _ in range(3):
+                    p.poison_hidden(0x7FC0)
+                    Y = p.run(Xd, Wd)
+                    assert np.array_equal(inputs.as_u16(Y.cpu()), outs[-1])
+                st = p.stats()
+                assert st.status == 0 and st.ready_ok == 1
+                for l in range(cfg.n_layers):
+                    assert st.units_done[l] == st.units[l]
+                p.close()
