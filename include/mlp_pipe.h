@@ -80,6 +80,21 @@ enum {
                                        before publishing (adversarial schedule for the protocol)     */
 #define MLP_FLAG_DEBUG_REVERSE 0x4u /* test hook: layer-1 units are handed out in reverse order       */
 #define MLP_FLAG_NO_W_EVICT_FIRST 0x8u /* do not tag weight loads L2 evict-first                      */
+#define MLP_FLAG_ACQUIRE_LOADS 0x40u /* consumer prologue polls every ready counter with ld.acquire.gpu (the literal
+                                       form) instead of ld.relaxed.gpu + one fence.acq_rel.gpu per group of counters;
+                                       also switches the scheduler's look-ahead fast path off                       */
+/* Measurement knobs, each REMOVES one ingredient of the protocol to price it (results may be wrong; tests use them
+ * only to show that the ingredient matters or what it costs): */
+#define MLP_FLAG_EXP_NO_ACQUIRE_FENCE 0x10u /* no fence.acq_rel.gpu after the relaxed polls of the activation loader */
+#define MLP_FLAG_EXP_NO_PROXY_FENCE   0x20u /* no fence.proxy.async between the acquire and the TMA loads of H       */
+#define MLP_FLAG_EXP_NO_FAST_PATH     0x80u /* the scheduler never pre-checks a unit's ready counters                */
+#define MLP_FLAG_EXP_NO_PREISSUE      0x100u /* the first weight / activation ring is not requested during setup     */
+#define MLP_FLAG_PDL 0x800u         /* SEQUENTIAL only: layers 2.. are launched as PROGRAMMATIC DEPENDENTS of the layer
+                                       before (cudaLaunchAttributeProgrammaticStreamSerialization; not in the paper, whose baseline
+                                       only removes launch bubbles with CUDA Graphs): their
+                                       CTAs start as SMs become free, set up and prefetch weights, and execute
+                                       griddepcontrol.wait before the first load of the previous layer's output.  A
+                                       stronger stream-ordered baseline than plain back-to-back launches.               */
 #define MLP_FLAG_AUTOTUNE 0x400u    /* measured plan search: the FIRST mlp_pipe_run on the handle (outside stream
                                        capture) tries the planner's candidate K-splits / ticket orders on the
                                        caller's buffers, timing each with the in-kernel clock, and keeps the

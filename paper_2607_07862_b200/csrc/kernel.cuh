@@ -67,6 +67,10 @@ static_assert(sizeof(UnitDesc) == 8, "UnitDesc is read as one 8-byte word");
 
 constexpr int kActNone = 0, kActRelu = 1, kActGeluTanh = 2;
 constexpr uint32_t kFlagTileMajor = 0x1u, kFlagDebugDelay = 0x2u, kFlagDebugReverse = 0x4u, kFlagNoEvictFirst = 0x8u;
+// measurement knobs (include/mlp_pipe.h MLP_FLAG_EXP_*): each removes or replaces one protocol ingredient
+constexpr uint32_t kFlagExpNoAcquireFence = 0x10u, kFlagExpNoProxyFence = 0x20u, kFlagAcquireLoads = 0x40u,
+                   kFlagExpNoFastPath = 0x80u, kFlagExpNoPreissue = 0x100u;
+constexpr uint32_t kFlagPdl = 0x800u;  // SEQUENTIAL: layer l+1 is launched as a programmatic dependent of layer l
 constexpr uint32_t kStatusFlagTimeout = 1u;
 
 struct LayerParams {
@@ -120,6 +124,7 @@ struct KernelParams {
     int w_group;        // weight K-blocks requested back to back
     int producer_ctas;  // CTAs with blockIdx.x < producer_ctas start at layer_begin, the rest one layer later
     int wait_flags;     // consumer prologue on/off
+    int pdl_wait;       // 1: launched as a programmatic dependent; the activation loader waits for the grid before
     uint32_t flags;
     unsigned long long* epoch_counter;  // += 1 per exiting CTA; epoch = value / gridDim.x
     uint32_t* status;
@@ -385,6 +390,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
 
     // ------------------------------------------------------------------ one-time setup
     if (threadIdx.x == 0) {
+        if (P.flags & kFlagPdl) grid_launch_dependents();
         // device-resident epoch: no per-run host state, so a captured graph can be replayed
         *s_epoch = ld_relaxed_gpu_u64(reinterpret_cast<const uint64_t*>(P.epoch_counter)) / gridDim.x;
         for (int l = P.layer_begin; l < P.layer_end; ++l) {
@@ -425,7 +431,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
         }
         fence_mbar_init();
         uint32_t pre_w = 0, pre_a = 0;
-        if (have && ((raw.x >> 16) & 0xffu) == kUnitMma && !(P.flags & 0x100u)) {
+        if (have && ((raw.x >> 16) & 0xffu) == kUnitMma && !(P.flags & kFlagExpNoPreissue)) {
             fence_proxy_async();  // the barrier inits (generic proxy) before the TMA unit's complete_tx on them
             const int tile = static_cast<int>(raw.x & 0xffffu), kb0 = static_cast<int>(raw.y & 0xffffu), kb1 = static_cast<int>(raw.y >> 16);
             const int n_blk = tile % P.layer[l0].n_blks, m_blk = tile / P.layer[l0].n_blks;
@@ -438,7 +444,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                     tma_load_2d_hint(smem_base + i * w_tile_bytes, &P.tm_w[l0], (kb0 + static_cast<int>(i)) * kTileK, n_blk * tile_n, bar_full + 8 * i, pol);
                 else tma_load_2d(smem_base + i * w_tile_bytes, &P.tm_w[l0], (kb0 + static_cast<int>(i)) * kTileK, n_blk * tile_n, bar_full + 8 * i);
             }
-            if (l0 == P.layer_begin) {  // input of the launch: nothing to wait for
+            if (l0 == P.layer_begin && !P.pdl_wait) {  // input of the launch: nothing to wait for
                 pre_a = static_cast<uint32_t>(min(a_stages, kb1 - kb0));
                 for (uint32_t i = 0; i < pre_a; ++i) {
                     mbar_arrive_expect_tx(bar_afull + 8 * i, a_tile_bytes);
@@ -514,7 +520,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                             fence_acq_rel_gpu();
                             u.acquired = 1;
                         }
-                    } else if (P.wait_flags && l > P.layer_begin && !(P.flags & 0x80u)) {
+                    } else if (P.wait_flags && l > P.layer_begin && !(P.flags & (kFlagExpNoFastPath | kFlagAcquireLoads))) {
                         // Consumer prologue, fast path (the prologue lives in the scheduler
                         // warp): one look at all ready counters under this unit's K range.  If every producer
                         // tile is already published -- the normal case, the scheduler runs a unit ahead --
@@ -604,9 +610,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                         const uint32_t full = bar_full + 8 * stage;
                         mbar_arrive_expect_tx(full, w_tile_bytes);
                         const uint32_t dst = smem_base + stage * w_tile_bytes;
-                        if (P.flags & 0x200u)  // EXPERIMENT: contiguous 16 KB tiles (timing only, wrong data)
-                            tma_load_2d_hint(dst, tm, 0, (u.n_blk * P.layer[u.layer].kb_total + kb) * tile_n, full, pol);
-                        else if (hint) tma_load_2d_hint(dst, tm, kb * kTileK, u.n_blk * tile_n, full, pol);
+                        if (hint) tma_load_2d_hint(dst, tm, kb * kTileK, u.n_blk * tile_n, full, pol);
                         else tma_load_2d(dst, tm, kb * kTileK, u.n_blk * tile_n, full);
                         if (++stage == static_cast<uint32_t>(stages)) { stage = 0; phase ^= 1; }
                     }
@@ -621,6 +625,13 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
             uint32_t stage = 0, phase = 0;
             unsigned long long stall = 0, polls = 0;
             bool aborted = false;
+            if (P.pdl_wait) {
+                // programmatic dependent launch (stronger SEQUENTIAL baseline): this grid was allowed to start while
+                // the grid of the layer before still runs; setup and the weight prefetch overlap its tail, and only
+                // here -- before the first read of what it wrote -- do we wait for its completion
+                grid_dependency_wait();
+                fence_proxy_async();
+            }
             for (uint32_t it = 0;; ++it) {
                 const uint32_t slot = it % kSchedSlots;
                 mbar_wait(bar_sfull + 8 * slot, (it / kSchedSlots) & 1);
@@ -658,7 +669,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                             pend_base = ready_upto;
 #pragma unroll
                             for (int i = 0; i < 8; ++i)
-                                v[i] = (pend_base + i < slice_end) ? ((P.flags & 0x40u) ? ld_acquire_gpu(ready + pend_base + i) : ld_relaxed_gpu(ready + pend_base + i)) : target - 1u;
+                                v[i] = (pend_base + i < slice_end) ? ((P.flags & kFlagAcquireLoads) ? ld_acquire_gpu(ready + pend_base + i) : ld_relaxed_gpu(ready + pend_base + i)) : target - 1u;
                         }
                         if (slice >= ready_upto) {
                             int n_ok = 0;
@@ -670,7 +681,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                                     const long long c0 = clock64();
                                     const uint64_t t0 = globaltimer_ns();
                                     uint32_t n = 0;
-                                    while (static_cast<int32_t>(ld_relaxed_gpu(ready + slice) - target) < 0) {
+                                    while (static_cast<int32_t>(((P.flags & kFlagAcquireLoads) ? ld_acquire_gpu(ready + slice) : ld_relaxed_gpu(ready + slice)) - target) < 0) {
                                         ++n;
                                         __nanosleep(32);
                                         if ((n & 255u) == 0) {
@@ -687,10 +698,10 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                                 }
                                 n_ok = 1;
                             }
-                            if (!(P.flags & 0x10u)) fence_acq_rel_gpu();
+                            if (!(P.flags & (kFlagExpNoAcquireFence | kFlagAcquireLoads))) fence_acq_rel_gpu();
                             // H was written through the generic proxy; the TMA below reads it through
                             // the async proxy
-                            if (!(P.flags & 0x20u)) fence_proxy_async();
+                            if (!(P.flags & kFlagExpNoProxyFence)) fence_proxy_async();
                             ready_upto = pend_base + n_ok;
                             pend_base = -1;
                         }

@@ -747,8 +747,15 @@ int launch(mlp_pipe* h, KernelParams& P, cudaStream_t s) {
     cfg.blockDim = dim3(kThreads);
     cfg.dynamicSmemBytes = h->smem_bytes;
     cfg.stream = s;
+    cudaLaunchAttribute attr[1];
     cfg.attrs = nullptr;
     cfg.numAttrs = 0;
+    if (P.pdl_wait) {  // programmatic dependent launch of layer l+1 on layer l (a stronger baseline than the paper's)
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+    }
     CUDA_TRY(h, cudaLaunchKernelEx(&cfg, mlp_pipe_kernel, P));
     return MLP_OK;
 }
@@ -887,10 +894,7 @@ int run_core(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStre
     KernelParams P = h->base;
     if ((rc = lookup_tmap(h, h->cache_x, &h->cache_x_next, X, h->M, h->widths[0], h->tile_m, &P.tm_a[0]))) return rc;
     for (int l = 0; l < h->L; ++l)
-        if (h->mode.flags & 0x200u) {  // EXPERIMENT: view W as [N K / 64 x 64]: a box is 16 KB of contiguous memory
-            if ((rc = lookup_tmap(h, h->cache_w[l], &h->cache_w_next[l], W[l], h->widths[l + 1] * (h->widths[l] / 64), 64, kTileN * h->n_sub, &P.tm_w[l])))
-                return rc;
-        } else if ((rc = lookup_tmap(h, h->cache_w[l], &h->cache_w_next[l], W[l], h->widths[l + 1], h->widths[l], kTileN * h->n_sub, &P.tm_w[l])))
+        if ((rc = lookup_tmap(h, h->cache_w[l], &h->cache_w_next[l], W[l], h->widths[l + 1], h->widths[l], kTileN * h->n_sub, &P.tm_w[l])))
             return rc;
     P.layer[h->L - 1].out = static_cast<__nv_bfloat16*>(Y);
 
@@ -914,6 +918,7 @@ int run_core(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStre
             P.m_off = 0;
             P.m_end = h->M;
             P.wait_flags = 0;
+            P.pdl_wait = (h->mode.flags & MLP_FLAG_PDL) && l > 0 ? 1 : 0;
             P.producer_ctas = h->grid;
             P.epoch_counter = h->epoch + l;
             P.stats = h->stats + static_cast<size_t>(l) * h->grid;
@@ -970,6 +975,16 @@ int last_span_us(mlp_pipe* h, double* out) {
 int autotune(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStream_t s) {
     int rc;
     CUDA_TRY(h, cudaStreamSynchronize(s));
+    // candidates are ranked by per-launch in-kernel spans, which overlap under programmatic dependent launch:
+    // search with plain stream order, run with PDL afterwards
+    const std::string key = plan_key(h);
+    const unsigned saved_flags = h->mode.flags;
+    h->mode.flags &= ~static_cast<unsigned>(MLP_FLAG_PDL);
+    struct Restore {
+        mlp_pipe* h;
+        unsigned f;
+        ~Restore() { h->mode.flags = f; }
+    } restore{h, saved_flags};
     Planner pl = make_planner(h);
     auto measure = [&](double* us) -> int {
         int r = install_plan(h);
@@ -1012,6 +1027,7 @@ int autotune(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStre
         }
         if (!improved) break;
     }
+    h->mode.flags = saved_flags;
     if ((rc = install_plan(h))) return rc;
     h->tuned_us = best_us;
     h->tuned = true;
@@ -1019,7 +1035,7 @@ int autotune(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStre
         std::lock_guard<std::mutex> lock(g_plan_mutex);
         std::vector<std::vector<int>> v(h->L);
         for (int l = 0; l < h->L; ++l) v[l] = h->bounds[l];
-        g_plan_cache[plan_key(h) + "#tuned"] = v;
+        g_plan_cache[key + "#tuned"] = v;
     }
     if (getenv("MLP_PIPE_DEBUG")) {
         fprintf(stderr, "[mlp_pipe] autotuned: %.1f us in-kernel span;", best_us);

@@ -101,6 +101,12 @@ __device__ __forceinline__ uint32_t atom_add_relaxed_gpu(uint32_t* p, uint32_t v
     return old;
 }
 
+// ------------------------------------------------------------------ programmatic dependent launch
+// wait: until the grid(s) this launch depends on have completed and their writes are visible;
+// launch_dependents: the next launch in the stream may start its CTAs as SMs become free.
+__device__ __forceinline__ void grid_dependency_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void grid_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // ------------------------------------------------------------------ TMA
 __device__ __forceinline__ void prefetch_tmap(const CUtensorMap* m) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(m)) : "memory");

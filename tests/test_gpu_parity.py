@@ -297,3 +297,38 @@ def test_autotune_keeps_results_exact_and_state_consistent():
                 for l in range(cfg.n_layers):
                     assert st.units_done[l] == st.units[l]
                 p.close()
+
+
+def test_literal_ld_acquire_polls():
+    """MLP_FLAG_ACQUIRE_LOADS: the consumer prologue polls with ld.acquire.gpu (BASELINE.json north_star's literal
+    wording) instead of relaxed polls + one acquire fence; same bits, poisoned H, adversarial delays."""
+    cfg = inputs.Config("acq", 64, (1024, 4096, 1024), B.MLP_ACT_RELU, "exact", 5)
+    X, Ws, outs, _ = oracle_outs(cfg)
+    Xd, Wd = X.cuda(), [w.cuda() for w in Ws]
+    for flags in (B.MLP_FLAG_ACQUIRE_LOADS, B.MLP_FLAG_ACQUIRE_LOADS | B.MLP_FLAG_DEBUG_DELAY):
+        p = B.MlpPipe(cfg.M, cfg.widths, cfg.act, B.make_mode(P, split_k=4, flags=flags))
+        for _ in range(10):
+            p.poison_hidden(0x7FC0)
+            Y = p.run(Xd, Wd)
+            assert np.array_equal(inputs.as_u16(Y.cpu()), outs[-1])
+        st = p.stats()
+        assert st.ready_ok == 1 and st.status == 0
+        p.close()
+    check(inputs.CONFIGS[1], B.make_mode(P, flags=B.MLP_FLAG_ACQUIRE_LOADS))
+
+
+def test_sequential_with_programmatic_dependent_launch():
+    """MLP_FLAG_PDL: layer l+1 starts while layer l still runs and waits (griddepcontrol.wait) before its first read
+    of H; results must be those of plain SEQUENTIAL, with H poisoned before every run."""
+    for cfg in (inputs.get_config(0, "exact"), inputs.Config("pdl_3l", 48, (256, 1024, 512, 256), B.MLP_ACT_RELU, "exact", 9)):
+        X, Ws, outs, _ = oracle_outs(cfg)
+        Xd, Wd = X.cuda(), [w.cuda() for w in Ws]
+        p = B.MlpPipe(cfg.M, cfg.widths, cfg.act, B.make_mode(S, flags=B.MLP_FLAG_PDL, split_k=2))
+        for _ in range(20):
+            p.poison_hidden(0x7FC0)
+            Y = p.run(Xd, Wd)
+            assert np.array_equal(inputs.as_u16(Y.cpu()), outs[-1])
+        st = p.stats()
+        assert st.ready_ok == 1 and st.status == 0
+        p.close()
+    check(inputs.CONFIGS[1], B.make_mode(S, flags=B.MLP_FLAG_PDL))
