@@ -329,15 +329,47 @@ def extras(torch, B, inputs, cfg, args, X, sets, Y, with_cpu=True):
     out = {}
     modes = {}
     tune = 0 if args.no_autotune else B.MLP_FLAG_AUTOTUNE
-    for name, mode in (("sequential", B.make_mode(B.MLP_SEQUENTIAL, stages=args.stages, flags=tune)),
-                       ("microbatch2", B.make_mode(B.MLP_MICROBATCH, chunks=2, stages=args.stages)),
-                       ("pipelined_sm_split_0.5", B.make_mode(B.MLP_CTA_PIPELINED, sm_split=0.5, stages=args.stages, flags=tune))):
-        if cfg.M % 2 and name == "microbatch2":
-            continue
+    cands = [("sequential", B.make_mode(B.MLP_SEQUENTIAL, stages=args.stages, flags=tune)),
+             ("sequential_pdl", B.make_mode(B.MLP_SEQUENTIAL, stages=args.stages, flags=tune | B.MLP_FLAG_PDL))]
+    for c in (2, 4, 8):   # BASELINE.json: sweep MICROBATCH chunks {2,4,8}
+        if cfg.M % c == 0:
+            cands.append((f"microbatch{c}", B.make_mode(B.MLP_MICROBATCH, chunks=c, stages=args.stages)))
+    cands.append(("pipelined_sm_split_0.5", B.make_mode(B.MLP_CTA_PIPELINED, sm_split=0.5, stages=args.stages, flags=tune)))
+    for name, mode in cands:
         p = B.MlpPipe(cfg.M, cfg.widths, cfg.act, mode)
         lat, _ = time_steps(torch, p, X, sets, Y, min(args.steps, 100), max(3, min(args.warmup, 10)))
         modes[name] = {"median_us": lat["median"], "p10_us": lat["p10"], "p90_us": lat["p90"]}
         p.close()
+    # the headline mode replayed from a CUDA graph ("can be captured by CUDA Graphs"): same kernel,
+    # launch issued by the graph instead of cudaLaunchKernelEx
+    try:
+        p = B.MlpPipe(cfg.M, cfg.widths, cfg.act, make_mode(B, args, cfg.n_layers))
+        s_cap = torch.cuda.Stream()
+        with torch.cuda.stream(s_cap):
+            for i in range(3):
+                p.run(X, sets[0], Y, stream=s_cap)      # tunes + encodes the tensor maps outside the capture
+            s_cap.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=s_cap):
+                p.run(X, sets[0], Y, stream=s_cap)
+        torch.cuda.synchronize()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(min(args.steps, 100))]
+        for _ in range(5):
+            g.replay()
+        torch.cuda.synchronize()
+        torch.cuda._sleep(2_000_000)
+        for a, b in ev:
+            a.record()
+            g.replay()
+            b.record()
+        torch.cuda.synchronize()
+        ts = sorted(a.elapsed_time(b) * 1e3 for a, b in ev)
+        modes["pipelined_cuda_graph_same_weights"] = {"median_us": ts[len(ts) // 2], "p10_us": ts[len(ts) // 10], "p90_us": ts[(9 * len(ts)) // 10],
+                                                      "note": "one weight set replayed: weights partly L2-resident, not comparable to the headline"}
+        del g
+        p.close()
+    except Exception as e:  # graph capture is an extra, never fatal for the bench line
+        modes["pipelined_cuda_graph_same_weights"] = {"error": str(e)[:200]}
     out["other_modes"] = modes
 
     # e2e: the same step through mlp_pipe_run_host -- pinned host X / W_l in, Y out, copies inside the timed region
