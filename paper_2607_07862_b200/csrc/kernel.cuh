@@ -83,6 +83,8 @@ struct LayerParams {
     int ticket_off;  // unit index of the first atomically drawn ticket (= units handed out statically)
     int act;       // activation on this layer's output
     int publish;   // 1 if a later layer consumes this layer's output
+    int static_sp;    // > 0: tickets t < grid of this layer are MMA units (tile t / static_sp, slice t % static_sp, equal
+                      // slices) -- lets a CTA decode its static first unit without reading the table
     int reduce_mode;  // kReduceNone (split == 1) | kReduceLastArriver | kReduceUnits
     int ready_inc;    // what one run adds to a tile's ready counter (1, or its number of reduce units)
     __nv_bfloat16* out;  // [M x N] row-major
@@ -315,6 +317,17 @@ __device__ __forceinline__ void drain_acc(uint32_t taddr, int total, uint32_t ba
     }
 }
 
+// Table entry of ticket t as the two words of a UnitDesc; computed when the layer's first tickets follow the
+// closed form (static_sp), else read.
+__device__ __forceinline__ uint2 unit_words(const LayerParams& L, uint32_t t, bool may_compute) {
+    if (may_compute && L.static_sp > 0) {
+        const uint32_t sp = static_cast<uint32_t>(L.static_sp), tile = t / sp, ks = t % sp;
+        const uint32_t a = ks * static_cast<uint32_t>(L.kb_total) / sp, b = (ks + 1) * static_cast<uint32_t>(L.kb_total) / sp;
+        return make_uint2(tile | (static_cast<uint32_t>(kUnitMma) << 16) | (ks << 24), a | (b << 16));
+    }
+    return __ldg(reinterpret_cast<const uint2*>(L.table) + t);
+}
+
 // Spin until *ctr has reached `target` (wrap-safe), then acquire.  Relaxed polls + one acquire fence =
 // acquire pattern.  Bounded: after timeout_ns (or when another waiter has already given up) the wait is
 // abandoned, the device status word records it and the caller carries on (output undefined, kernel ends).
@@ -373,7 +386,8 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
     volatile uint32_t* s_tmem = reinterpret_cast<volatile uint32_t*>(ctrl + kBarBytes + sizeof(UnitInfo) * kSchedSlots);
     volatile uint32_t* s_last = s_tmem + 1;
     volatile unsigned long long* s_epoch = reinterpret_cast<volatile unsigned long long*>(s_tmem + 2);
-    volatile uint32_t* s_pre = s_tmem + 4;  // [0] weight / [1] activation K-blocks of the first unit requested during setup
+    volatile uint32_t* s_pre = s_tmem + 4;  // [0] weight / [1] activation K-blocks of the first unit requested during setup,
+                                            // [2] 1 if the first unit already sits in slot 0 of the scheduler ring
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
@@ -398,6 +412,21 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
             prefetch_tmap(&P.tm_a[l]);
         }
     }
+    if (warp == 1) {
+        // All mbarriers live in one array of 8-byte slots; the 32 lanes of the weight-loader warp initialise them in
+        // parallel (92 serial mbarrier.init cost ~1 us at the head of every CTA), arrival counts by slot range.
+        constexpr int kNumBars = 4 * kMaxStages + 2 * kMaxAccStages + 3 * kSchedSlots;
+        for (int b = lane; b < kNumBars; b += 32) {
+            uint32_t count = 1;
+            if (b >= 4 * kMaxStages + kMaxAccStages && b < 4 * kMaxStages + 2 * kMaxAccStages) count = kEpiThreads;                   // tempty
+            if (b >= 4 * kMaxStages + 2 * kMaxAccStages + kSchedSlots && b < 4 * kMaxStages + 2 * kMaxAccStages + 2 * kSchedSlots)
+                count = 3 + kEpiThreads;                                                                                              // sempty
+            mbar_init(bar_full + 8 * b, count);
+        }
+        fence_mbar_init();
+        fence_proxy_async();  // the inits (generic proxy) before the TMA unit's complete_tx on them
+        __syncwarp();
+    }
     if (threadIdx.x == 32) {
         // This thread is the weight loader.  The first unit of the CTA is static (same rule as in the
         // scheduler below), so its first ring of weight tiles -- and, if it has no producers, of activation
@@ -411,24 +440,9 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
         }
         const bool have = sid < static_cast<uint32_t>(P.layer[l0].units);
         uint2 raw = make_uint2(0u, 0u);
-        if (have) raw = __ldg(reinterpret_cast<const uint2*>(P.layer[l0].table) + sid);  // in flight during the inits
-        for (int s = 0; s < stages; ++s) {
-            mbar_init(bar_full + 8 * s, 1);
-            mbar_init(bar_empty + 8 * s, 1);
-        }
-        for (int s = 0; s < a_stages; ++s) {
-            mbar_init(bar_afull + 8 * s, 1);
-            mbar_init(bar_aempty + 8 * s, 1);
-        }
-        for (int i = 0; i < kMaxAccStages; ++i) {
-            mbar_init(bar_tfull + 8 * i, 1);
-            mbar_init(bar_tempty + 8 * i, kEpiThreads);
-        }
-        for (int i = 0; i < kSchedSlots; ++i) {
-            mbar_init(bar_sfull + 8 * i, 1);
-            mbar_init(bar_sempty + 8 * i, 3 + kEpiThreads);
-            mbar_init(bar_wtaken + 8 * i, 1);
-        }
+        prefetch_tmap(&P.tm_w[l0]);
+        prefetch_tmap(&P.tm_a[l0]);
+        if (have) raw = unit_words(P.layer[l0], sid, true);
         fence_mbar_init();
         uint32_t pre_w = 0, pre_a = 0;
         if (have && ((raw.x >> 16) & 0xffu) == kUnitMma && !(P.flags & kFlagExpNoPreissue)) {
@@ -445,7 +459,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 else tma_load_2d(smem_base + i * w_tile_bytes, &P.tm_w[l0], (kb0 + static_cast<int>(i)) * kTileK, n_blk * tile_n, bar_full + 8 * i);
             }
             if (l0 == P.layer_begin && !P.pdl_wait) {  // input of the launch: nothing to wait for
-                pre_a = static_cast<uint32_t>(min(a_stages, kb1 - kb0));
+                pre_a = static_cast<uint32_t>(min(min(a_stages, stages), kb1 - kb0));
                 for (uint32_t i = 0; i < pre_a; ++i) {
                     mbar_arrive_expect_tx(bar_afull + 8 * i, a_tile_bytes);
                     tma_load_2d(a_ring + i * a_tile_bytes, &P.tm_a[l0], (kb0 + static_cast<int>(i)) * kTileK, P.m_off + m_blk * tile_m, bar_afull + 8 * i);
@@ -454,6 +468,25 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
         }
         s_pre[0] = pre_w;
         s_pre[1] = pre_a;
+        // ... and the unit itself goes into slot 0 of the scheduler ring right away, so that after the CTA-wide sync
+        // the MMA / loader / epilogue warps start on it without waiting for the scheduler warp
+        s_pre[2] = have ? 1u : 0u;
+        if (have) {
+            UnitInfo u;
+            u.layer = l0;
+            u.tile = static_cast<int>(raw.x & 0xffffu);
+            u.kind = static_cast<int>((raw.x >> 16) & 0xffu);
+            u.ks = static_cast<int>(raw.x >> 24);
+            u.kb0 = static_cast<int>(raw.y & 0xffffu);
+            u.kb1 = static_cast<int>(raw.y >> 16);
+            u.m_blk = u.tile / P.layer[l0].n_blks;
+            u.n_blk = u.tile % P.layer[l0].n_blks;
+            u.valid = 1;
+            u.acquired = 0;  // a consumer-first or reduce unit polls for itself
+            u.pad_[0] = u.pad_[1] = 0;
+            ring[0] = u;
+            mbar_arrive(bar_sfull);  // slot 0 (release: the slot is visible to the waiters)
+        }
     }
     if (warp == 3) {
         tmem_alloc(smem_u32(const_cast<uint32_t*>(s_tmem)), tmem_cols);
@@ -483,6 +516,12 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
             }
             uint32_t it = 0;
             bool finished = false;
+            if (s_pre[2]) {  // the static first unit was published by the weight loader during setup
+                use_static = false;
+                done[l] = 1;
+                it = 1;
+                my_stats->ts[2] = globaltimer_ns();
+            }
             while (!finished) {
                 UnitInfo u;
                 u.valid = 0;
@@ -503,7 +542,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                         ++l;
                         continue;
                     }
-                    const uint2 raw = __ldg(reinterpret_cast<const uint2*>(L.table) + t);
+                    const uint2 raw = unit_words(L, t, it == 0);
                     u.layer = l;
                     u.tile = static_cast<int>(raw.x & 0xffffu);
                     u.kind = static_cast<int>((raw.x >> 16) & 0xffu);

@@ -669,6 +669,16 @@ int build_base_params(mlp_pipe* h) {
         Lp.act = l < h->L - 1 ? h->act : kActNone;
         Lp.publish = l < h->L - 1 ? 1 : 0;
         Lp.reduce_mode = h->reduce_mode[l];
+        {   // do the first `grid` tickets follow the closed form (tile-major, equal slices)?
+            const int sp = h->split[l], n = std::min<int>(h->grid, static_cast<int>(h->table[l].size()));
+            bool ok = sp <= 255;
+            for (int t = 0; t < n && ok; ++t) {
+                const UnitDesc& d = h->table[l][t];
+                const int ks = t % sp;
+                ok = d.kind == kUnitMma && d.tile == t / sp && d.ks == ks && d.a == ks * Lp.kb_total / sp && d.b == (ks + 1) * Lp.kb_total / sp;
+            }
+            Lp.static_sp = ok ? sp : 0;
+        }
         Lp.ready_inc = h->ready_inc[l];
         Lp.table = h->d_table[l];
         Lp.out = l < h->L - 1 ? h->H[l] : nullptr;  // last layer: caller's Y, patched per run
