@@ -335,10 +335,13 @@ def extras(torch, B, inputs, cfg, args, X, sets, Y, with_cpu=True):
         if cfg.M % c == 0:
             cands.append((f"microbatch{c}", B.make_mode(B.MLP_MICROBATCH, chunks=c, stages=args.stages)))
     cands.append(("pipelined_sm_split_0.5", B.make_mode(B.MLP_CTA_PIPELINED, sm_split=0.5, stages=args.stages, flags=tune)))
+    # the paper's literal scoreboard + work-queue protocol as an A/B of the consumer prologue
+    cands.append(("pipelined_workqueue", B.make_mode(B.MLP_CTA_PIPELINED, stages=args.stages, flags=tune | B.MLP_FLAG_WORKQUEUE)))
     for name, mode in cands:
         p = B.MlpPipe(cfg.M, cfg.widths, cfg.act, mode)
         lat, _ = time_steps(torch, p, X, sets, Y, min(args.steps, 100), max(3, min(args.warmup, 10)))
-        modes[name] = {"median_us": lat["median"], "p10_us": lat["p10"], "p90_us": lat["p90"]}
+        modes[name] = {"median_us": lat["median"], "p10_us": lat["p10"], "p90_us": lat["p90"],
+                       "flag_stall_cycles_max": int(p.stats().flag_stall_cycles_max)}
         p.close()
     # the headline mode replayed from a CUDA graph ("can be captured by CUDA Graphs"): same kernel,
     # launch issued by the graph instead of cudaLaunchKernelEx

@@ -95,6 +95,12 @@ enum {
                                        CTAs start as SMs become free, set up and prefetch weights, and execute
                                        griddepcontrol.wait before the first load of the previous layer's output.  A
                                        stronger stream-ordered baseline than plain back-to-back launches.               */
+#define MLP_FLAG_WORKQUEUE 0x1000u  /* CTA_PIPELINED only: the paper's literal protocol instead of polled ready
+                                       counters.  Producer epilogue: dependency array -> scoreboard update -> push of the
+                                       now-ready consumer units into a work queue; consumer prologue: a ticket is a queue
+                                       POSITION, the CTA spins until an entry appears there and remaps its unit to it (units
+                                       run in the order in which they became ready; the weights of a unit cannot be
+                                       prefetched before the pop).  Split tiles are summed by the last-arriving slice.       */
 #define MLP_FLAG_AUTOTUNE 0x400u    /* measured plan search: the FIRST mlp_pipe_run on the handle (outside stream
                                        capture) tries the planner's candidate K-splits / ticket orders on the
                                        caller's buffers, timing each with the in-kernel clock, and keeps the

@@ -70,6 +70,7 @@ constexpr uint32_t kFlagTileMajor = 0x1u, kFlagDebugDelay = 0x2u, kFlagDebugReve
 // measurement knobs (include/mlp_pipe.h MLP_FLAG_EXP_*): each removes or replaces one protocol ingredient
 constexpr uint32_t kFlagExpNoAcquireFence = 0x10u, kFlagExpNoProxyFence = 0x20u, kFlagAcquireLoads = 0x40u,
                    kFlagExpNoFastPath = 0x80u, kFlagExpNoPreissue = 0x100u;
+constexpr uint32_t kFlagWorkQueue = 0x1000u;  // consumers pop ready units from a work queue instead of polling ready counters
 constexpr uint32_t kFlagPdl = 0x800u;  // SEQUENTIAL: layer l+1 is launched as a programmatic dependent of layer l
 constexpr uint32_t kStatusFlagTimeout = 1u;
 
@@ -93,6 +94,17 @@ struct LayerParams {
     uint32_t* arrive;    // [tiles] monotone split-K arrival counters
     uint32_t* ready;     // [tiles] monotone ready counters, tile = m_blk * n_blks + n_blk
     const UnitDesc* table;  // [units] ticket -> unit
+    // ---- the paper's literal protocol, MLP_FLAG_WORKQUEUE: dependency array -> scoreboard -> work queue.
+    // A GROUP of this layer = its units with the same (M-block, K-slice): they depend on the same producer tiles.
+    int use_queue;               // 1: tickets of this layer index its work queue (unit order = order in which groups become ready)
+    int group_units;             // units per group (= N-tiles per M-block)
+    uint32_t* scoreboard;        // [groups] monotone: += 1 per finished producer tile the group depends on
+    uint32_t* qtail;             // 1 monotone counter: next free queue slot
+    uint32_t* queue;             // [units] slot = (epoch tag << 16) | table index
+    const uint16_t* dep_count;   // [groups] producer tiles a group depends on
+    const uint16_t* qorder;      // [groups][group_units] table indices of a group's units
+    const uint16_t* dep_off;     // [tiles of the layer BEFORE + 1] CSR offsets into dep_list: "dependency array" of a producer tile
+    const uint16_t* dep_list;    // groups of THIS layer that depend on that producer tile
 };
 
 struct CtaStats {
@@ -317,6 +329,10 @@ __device__ __forceinline__ void drain_acc(uint32_t taddr, int total, uint32_t ba
     }
 }
 
+__device__ __forceinline__ void st_relaxed_gpu(uint32_t* p, uint32_t v) {
+    asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
 // Table entry of ticket t as the two words of a UnitDesc; computed when the layer's first tickets follow the
 // closed form (static_sp), else read.
 __device__ __forceinline__ uint2 unit_words(const LayerParams& L, uint32_t t, bool may_compute) {
@@ -438,7 +454,8 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
             l0 = P.layer_begin + 1;
             sid = blockIdx.x - P.producer_ctas;
         }
-        const bool have = sid < static_cast<uint32_t>(P.layer[l0].units);
+        const bool have = sid < static_cast<uint32_t>(P.layer[l0].units) &&
+                          !(P.layer[l0].use_queue && P.wait_flags && l0 > P.layer_begin);  // (a queue-mode unit is unknown until popped)
         uint2 raw = make_uint2(0u, 0u);
         prefetch_tmap(&P.tm_w[l0]);
         prefetch_tmap(&P.tm_a[l0]);
@@ -505,6 +522,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
         if (lane == 0) {
             uint32_t done[kMaxLayers];
             for (int l = 0; l < kMaxLayers; ++l) done[l] = 0;
+            unsigned long long q_stall = 0, q_polls = 0;
             int l = P.layer_begin;
             // the first unit of a CTA is static (its rank among the CTAs that start on the same layer):
             // no atomic round trip before the first weight load
@@ -542,7 +560,42 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                         ++l;
                         continue;
                     }
-                    const uint2 raw = unit_words(L, t, it == 0);
+                    uint2 raw;
+                    bool popped = false;
+                    if (L.use_queue && P.wait_flags && l > P.layer_begin) {
+                        // Consumer prologue of the paper's protocol (PAPER.md:95 step (5)): ticket t is a
+                        // POSITION in the work queue; spin until a producer has pushed an entry there, then remap
+                        // the unit ("tile id") to what the entry names.  Entries appear in the order in which groups
+                        // of units became ready, so the unit -- and with it the weights to prefetch -- is not known
+                        // before the pop.
+                        const uint32_t tag = static_cast<uint32_t>(epoch + 1ull) & 0xffffu;
+                        uint32_t v = ld_relaxed_gpu(L.queue + t);
+                        if ((v >> 16) != tag) {
+                            const long long c0 = clock64();
+                            const uint64_t t0 = globaltimer_ns();
+                            uint32_t n = 0;
+                            bool gave_up = false;
+                            while (((v = ld_relaxed_gpu(L.queue + t)) >> 16) != tag) {
+                                __nanosleep(32);
+                                if ((++n & 255u) == 0) {
+                                    if (ld_relaxed_gpu(P.status) != 0) { gave_up = true; break; }
+                                    if (globaltimer_ns() - t0 > P.timeout_ns) {
+                                        atomicCAS(P.status, 0u, kStatusFlagTimeout);
+                                        gave_up = true;
+                                        break;
+                                    }
+                                }
+                            }
+                            q_stall += static_cast<unsigned long long>(clock64() - c0);
+                            q_polls += n;
+                            if (gave_up) v = t;  // watchdog: fall back to the static order so that the kernel terminates
+                        }
+                        fence_acq_rel_gpu();  // acquire: the pusher released after the last producer tile of the group
+                        raw = __ldg(reinterpret_cast<const uint2*>(L.table) + (v & 0xffffu));
+                        popped = true;
+                    } else {
+                        raw = unit_words(L, t, it == 0);
+                    }
                     u.layer = l;
                     u.tile = static_cast<int>(raw.x & 0xffffu);
                     u.kind = static_cast<int>((raw.x >> 16) & 0xffu);
@@ -552,7 +605,9 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                     u.m_blk = u.tile / L.n_blks;
                     u.n_blk = u.tile % L.n_blks;
                     u.valid = 1;
-                    if (u.kind == kUnitReduce) {
+                    if (popped) {
+                        u.acquired = 1;
+                    } else if (u.kind == kUnitReduce) {
                         // fast path of a reduce unit: all slices of its tile have already arrived
                         const uint32_t target = static_cast<uint32_t>((epoch + 1ull) * static_cast<unsigned long long>(L.split));
                         if (static_cast<int32_t>(ld_relaxed_gpu(L.arrive + u.tile) - target) >= 0) {
@@ -594,6 +649,10 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 ++it;
             }
             for (int l2 = 0; l2 < kMaxLayers; ++l2) P.stats[blockIdx.x].units[l2] = done[l2];
+            if (P.flags & kFlagWorkQueue) {  // (the activation loader never polls in this mode)
+                my_stats->stall_cycles = q_stall;
+                my_stats->polls = q_polls;
+            }
         }
     } else if (warp == 1) {
         // ===== W loader
@@ -750,8 +809,10 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                     if (++stage == static_cast<uint32_t>(a_stages)) { stage = 0; phase ^= 1; }
                 }
             }
-            P.stats[blockIdx.x].stall_cycles = stall;
-            P.stats[blockIdx.x].polls = polls;
+            if (!(P.flags & kFlagWorkQueue)) {
+                P.stats[blockIdx.x].stall_cycles = stall;
+                P.stats[blockIdx.x].polls = polls;
+            }
         }
     } else if (warp == 3) {
         // ===== MMA issuer (steps a2, a6)
@@ -907,6 +968,25 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 }
                 bar_sync(1, kEpiThreads);
                 if (r == 0) red_release_gpu_add(L.ready + u.tile, 1u);  // release: orders the tile before the counter
+                if (r == 0 && P.wait_flags && u.layer + 1 < P.layer_end && P.layer[u.layer + 1].use_queue) {
+                    // Producer epilogue of the paper's protocol (PAPER.md:95 steps (2)-(4)): look the tile up in the
+                    // dependency array, update the scoreboard entry of every group that depends on it, and push the
+                    // units of a group whose last dependency this was into the consumer's work queue.
+                    const LayerParams& Ln = P.layer[u.layer + 1];
+                    const uint32_t tag = static_cast<uint32_t>(epoch + 1ull) & 0xffffu;
+                    for (int k = __ldg(Ln.dep_off + u.tile); k < static_cast<int>(__ldg(Ln.dep_off + u.tile + 1)); ++k) {
+                        const uint32_t g = __ldg(Ln.dep_list + k);
+                        const uint32_t target = static_cast<uint32_t>((epoch + 1ull) * __ldg(Ln.dep_count + g));
+                        // acq_rel: releases this tile, and (for the last arrival) acquires every other producer's tile
+                        if (atom_add_acq_rel_gpu(Ln.scoreboard + g, 1u) + 1u == target) {
+                            const uint32_t base = atom_add_relaxed_gpu(Ln.qtail, static_cast<uint32_t>(Ln.group_units)) -
+                                                  static_cast<uint32_t>(epoch * static_cast<unsigned long long>(Ln.units));
+                            fence_acq_rel_gpu();  // release pattern for the slot stores below
+                            for (int i = 0; i < Ln.group_units; ++i)
+                                st_relaxed_gpu(Ln.queue + base + i, (tag << 16) | __ldg(Ln.qorder + g * Ln.group_units + i));
+                        }
+                    }
+                }
             }
             if (it == 0 && r == 0) my_stats->ts[6] = globaltimer_ns();
             if (it < kUnitTrace && r == 0) my_stats->unit_ts[it][3] = globaltimer_ns();

@@ -55,6 +55,13 @@ struct mlp_pipe {
     UnitDesc* d_table[kMaxLayers] = {nullptr};  // the same on the device
     int tiles[kMaxLayers] = {0};
     double model_us = 0.0;  // the planner's estimate of the launch(es)
+    // MLP_FLAG_WORKQUEUE: per consumer layer l >= 1 one device block [scoreboard | qtail | queue] (u32, zeroed with the
+    // counters) and one block of u16 tables [dep_count | qorder | dep_off | dep_list]
+    uint32_t* q_state[kMaxLayers] = {nullptr};
+    size_t q_state_words[kMaxLayers] = {0};
+    uint16_t* q_tables[kMaxLayers] = {nullptr};
+    int q_groups[kMaxLayers] = {0};
+    std::vector<uint16_t> q_dep_count[kMaxLayers];
     int kb_min = 0, kb_floor = 0;   // smallest K-slice the planner considers / allows
     bool fixed_split[kMaxLayers] = {false};  // the caller pinned this layer's split
     size_t table_cap[kMaxLayers] = {0};      // entries allocated for d_table[l]
@@ -213,6 +220,7 @@ struct Planner {
     }
     int reduce_mode_for(int sp) const {
         if (sp <= 1) return kReduceNone;
+        if (h->mode.flags & MLP_FLAG_WORKQUEUE) return kReduceLastArriver;  // queue entries are MMA units only
         // the last arriver sums sp partials on ONE SM, kGather slices x 16 token columns per dependent round
         // trip: fine for decode-sized tiles (<= 2 trips), a long serial tail otherwise
         const int trips = h->n_sub * (h->tile_m / 16) * ((sp + kGather - 1) / kGather);
@@ -681,6 +689,20 @@ int build_base_params(mlp_pipe* h) {
         }
         Lp.ready_inc = h->ready_inc[l];
         Lp.table = h->d_table[l];
+        Lp.use_queue = 0;
+        if (h->q_state[l]) {
+            const int n_blks = h->tiles[l] / h->m_blks, groups = h->q_groups[l], units = static_cast<int>(h->table[l].size());
+            Lp.use_queue = 1;
+            Lp.group_units = n_blks;
+            Lp.scoreboard = h->q_state[l];
+            Lp.qtail = h->q_state[l] + round_up(groups, 32);
+            Lp.queue = Lp.qtail + 32;
+            Lp.dep_count = h->q_tables[l];
+            Lp.qorder = Lp.dep_count + groups;
+            Lp.dep_off = Lp.qorder + static_cast<size_t>(groups) * n_blks;
+            Lp.dep_list = Lp.dep_off + h->tiles[l - 1] + 1;
+            (void)units;
+        }
         Lp.out = l < h->L - 1 ? h->H[l] : nullptr;  // last layer: caller's Y, patched per run
         Lp.ws = h->ws[l];
         Lp.ticket = h->ticket[l];
@@ -713,6 +735,8 @@ int build_base_params(mlp_pipe* h) {
 
 int reset_state(mlp_pipe* h, cudaStream_t s) {
     CUDA_TRY(h, cudaMemsetAsync(h->counters, 0, h->counters_words * sizeof(uint32_t), s));
+    for (int l = 0; l < kMaxLayers; ++l)
+        if (h->q_state[l]) CUDA_TRY(h, cudaMemsetAsync(h->q_state[l], 0, h->q_state_words[l] * sizeof(uint32_t), s));
     CUDA_TRY(h, cudaMemsetAsync(h->epoch, 0, kMaxLayers * sizeof(unsigned long long), s));
     CUDA_TRY(h, cudaMemsetAsync(h->status, 0, sizeof(uint32_t), s));
     CUDA_TRY(h, cudaMemsetAsync(h->stats, 0, sizeof(CtaStats) * kMaxLayers * h->grid, s));
@@ -790,6 +814,57 @@ int install_plan(mlp_pipe* h) {
             h->ws[l] = nullptr;
             h->ws_cap[l] = ws_bytes + ws_bytes / 4;
             CUDA_TRY(h, cudaMalloc(&h->ws[l], h->ws_cap[l]));
+        }
+    }
+    for (int l = 0; l < kMaxLayers; ++l) {
+        if (h->q_state[l]) CUDA_TRY(h, cudaFree(h->q_state[l]));
+        if (h->q_tables[l]) CUDA_TRY(h, cudaFree(h->q_tables[l]));
+        h->q_state[l] = nullptr;
+        h->q_tables[l] = nullptr;
+        h->q_groups[l] = 0;
+    }
+    if ((h->mode.flags & MLP_FLAG_WORKQUEUE) && h->mode.kind == MLP_CTA_PIPELINED) {
+        // The paper's data structures for every consumer layer l: groups g = (M-block, K-slice);
+        // dependency array of producer tile (m, j) = the groups of M-block m whose K range covers the columns of j;
+        // scoreboard[g] counts finished dependencies; the queue receives the units of a group when the count is full.
+        const int tn = kTileN * h->n_sub;
+        for (int l = 1; l < h->L; ++l) {
+            const int sp = h->split[l], n_blks = h->tiles[l] / h->m_blks, n_prev = h->tiles[l - 1] / h->m_blks;
+            const int groups = h->m_blks * sp, units = static_cast<int>(h->table[l].size());
+            if (units != h->tiles[l] * sp || units > 65535 || groups > 65535)
+                return fail(h, MLP_ERR_UNSUPPORTED, "MLP_FLAG_WORKQUEUE: layer %d has %d tickets (reduce units or > 65535)", l, units);
+            std::vector<uint16_t> dep_count(groups), qorder(static_cast<size_t>(groups) * n_blks), dep_off, dep_list;
+            std::vector<int> j0(sp), j1(sp);
+            for (int ks = 0; ks < sp; ++ks) {
+                j0[ks] = (h->bounds[l][ks] * kTileK) / tn;
+                j1[ks] = std::min(n_prev - 1, ((h->bounds[l][ks + 1] - 1) * kTileK) / tn);
+            }
+            for (int m = 0; m < h->m_blks; ++m)
+                for (int ks = 0; ks < sp; ++ks) dep_count[m * sp + ks] = static_cast<uint16_t>(j1[ks] - j0[ks] + 1);
+            for (int i = 0; i < units; ++i) {
+                const UnitDesc& d = h->table[l][i];
+                const int m = d.tile / n_blks, nb = d.tile % n_blks;
+                qorder[static_cast<size_t>(m * sp + d.ks) * n_blks + nb] = static_cast<uint16_t>(i);
+            }
+            for (int m = 0; m < h->m_blks; ++m)
+                for (int j = 0; j < n_prev; ++j) {
+                    dep_off.push_back(static_cast<uint16_t>(dep_list.size()));
+                    for (int ks = 0; ks < sp; ++ks)
+                        if (j0[ks] <= j && j <= j1[ks]) dep_list.push_back(static_cast<uint16_t>(m * sp + ks));
+                }
+            dep_off.push_back(static_cast<uint16_t>(dep_list.size()));
+            if (dep_list.size() > 65535) return fail(h, MLP_ERR_UNSUPPORTED, "MLP_FLAG_WORKQUEUE: dependency array too large");
+            std::vector<uint16_t> all;
+            all.insert(all.end(), dep_count.begin(), dep_count.end());
+            all.insert(all.end(), qorder.begin(), qorder.end());
+            all.insert(all.end(), dep_off.begin(), dep_off.end());
+            all.insert(all.end(), dep_list.begin(), dep_list.end());
+            CUDA_TRY(h, cudaMalloc(&h->q_tables[l], all.size() * sizeof(uint16_t)));
+            CUDA_TRY(h, cudaMemcpy(h->q_tables[l], all.data(), all.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
+            h->q_state_words[l] = static_cast<size_t>(round_up(groups, 32)) + 32 + round_up(units, 32);
+            CUDA_TRY(h, cudaMalloc(&h->q_state[l], h->q_state_words[l] * sizeof(uint32_t)));
+            h->q_groups[l] = groups;
+            h->q_dep_count[l] = dep_count;
         }
     }
     int rc = reset_state(h, nullptr);
@@ -1217,6 +1292,22 @@ int mlp_pipe_stats(mlp_pipe* h, mlp_stats* out, size_t bytes) {
             ok = ok && rd[t] == (l < h->L - 1 ? static_cast<uint32_t>(e * h->ready_inc[l]) : 0u);
         }
     }
+    for (int l = 1; l < h->L && ok; ++l) {  // work-queue protocol state: full scoreboards, every slot handed out
+        if (!h->q_state[l]) continue;
+        std::vector<uint32_t> q(h->q_state_words[l]);
+        CUDA_TRY(h, cudaMemcpy(q.data(), h->q_state[l], q.size() * sizeof(uint32_t), cudaMemcpyDeviceToHost));
+        const unsigned long long e = ep[0] / h->grid;
+        const int groups = h->q_groups[l], units = static_cast<int>(h->table[l].size());
+        for (int g = 0; g < groups && ok; ++g) ok = q[g] == static_cast<uint32_t>(e * h->q_dep_count[l][g]);
+        ok = ok && q[round_up(groups, 32)] == static_cast<uint32_t>(e * units);
+        const uint32_t tag = static_cast<uint32_t>(e) & 0xffffu;
+        std::vector<char> seen(units, 0);
+        for (int i = 0; i < units && ok && e > 0; ++i) {
+            const uint32_t v = q[round_up(groups, 32) + 32 + i];
+            ok = (v >> 16) == tag && (v & 0xffffu) < static_cast<uint32_t>(units) && !seen[v & 0xffffu];
+            if (ok) seen[v & 0xffffu] = 1;
+        }
+    }
     st.ready_ok = ok ? 1u : 0u;
     memcpy(out, &st, std::min(bytes, sizeof st));
     if (st.status != 0) {
@@ -1245,6 +1336,8 @@ void mlp_pipe_destroy(mlp_pipe* h) {
         if (h->H[l]) cudaFree(h->H[l]);
         if (h->ws[l]) cudaFree(h->ws[l]);
         if (h->d_table[l]) cudaFree(h->d_table[l]);
+        if (h->q_state[l]) cudaFree(h->q_state[l]);
+        if (h->q_tables[l]) cudaFree(h->q_tables[l]);
         if (h->stage_W[l]) cudaFree(h->stage_W[l]);
     }
     if (h->counters) cudaFree(h->counters);

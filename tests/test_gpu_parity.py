@@ -332,3 +332,37 @@ def test_sequential_with_programmatic_dependent_launch():
         assert st.ready_ok == 1 and st.status == 0
         p.close()
     check(inputs.CONFIGS[1], B.make_mode(S, flags=B.MLP_FLAG_PDL))
+
+
+WQ = B.MLP_FLAG_WORKQUEUE
+
+
+@pytest.mark.parametrize("flags", [WQ, WQ | B.MLP_FLAG_DEBUG_DELAY, WQ | B.MLP_FLAG_DEBUG_REVERSE | B.MLP_FLAG_DEBUG_DELAY])
+@pytest.mark.parametrize("sm_split", [1.0, 0.5])
+def test_workqueue_protocol_exact_with_poison(flags, sm_split):
+    """The paper's literal protocol: dependency array -> scoreboard -> work queue -> consumer pops and
+    remaps its unit.  Exact-mode bits under delayed / reversed producers with H poisoned before every run; afterwards
+    every scoreboard entry is full and the queue holds every unit exactly once."""
+    cfg = inputs.Config("wq", 64, (1024, 4096, 1024), B.MLP_ACT_RELU, "exact", 5)
+    X, Ws, outs, _ = oracle_outs(cfg)
+    p = B.MlpPipe(cfg.M, cfg.widths, cfg.act, B.make_mode(P, sm_split=sm_split, split_k=4, flags=flags))
+    Xd, Wd = X.cuda(), [w.cuda() for w in Ws]
+    for _ in range(20):
+        p.poison_hidden(0x7FC0)
+        Y = p.run(Xd, Wd)
+        assert np.array_equal(inputs.as_u16(Y.cpu()), outs[-1])
+    st = p.stats()
+    assert st.ready_ok == 1 and st.runs == 20 and st.status == 0
+    p.close()
+
+
+def test_workqueue_protocol_on_baseline_configs():
+    """Same protocol on BASELINE.json shapes: cfg 0 (both distributions), cfg 1 every element, the 4-layer chain (every
+    layer pair linked by its own scoreboard + queue) and M > 256 (several M-blocks = several groups per K-slice)."""
+    check(inputs.get_config(0, "exact"), B.make_mode(P, flags=WQ))
+    check(inputs.get_config(0), B.make_mode(P, flags=WQ))
+    check(inputs.CONFIGS[1], B.make_mode(P, flags=WQ))
+    check(inputs.Config("wq_m320", 320, (256, 512, 256), 1, "exact", 3), B.make_mode(P, flags=WQ, split_k=2, tile_m=64))
+    check(inputs.Config("wq_3l", 48, (256, 1024, 512, 256), B.MLP_ACT_RELU, "exact", 9), B.make_mode(P, flags=WQ))
+    err, st = sampled_rows_check(4, B.make_mode(P, flags=WQ), rows=[0, 31, 77, 127])
+    assert st.n_layers == 4
