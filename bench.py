@@ -240,7 +240,7 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": med, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": sum(ts) / len(ts) * scale / 1e3, "higher_is_better": False, "scaling": "weak",
         "vs_baseline": None, "dtype": "bf16 in/out, fp32 accumulate", "data": "synthetic",
-        "config": {"workload": f"BASELINE.json configs[{args.config}]: {cfg.name} M={cfg.M} widths={list(cfg.widths)}"},
+        "config": {"workload": f"BASELINE.json configs[{args.config}]: {cfg.name} M={cfg.M} widths={list(cfg.widths)} act={cfg.act}"},
         "cpu_baseline": {"value": med, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": med, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
