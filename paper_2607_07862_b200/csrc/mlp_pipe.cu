@@ -534,9 +534,17 @@ void resolve(mlp_pipe* h) {
     }
     // Weight rows per unit: 256 (two MMAs per K step that share the activation tile) once the activation
     // tile is large enough for its L2 traffic to matter and two accumulators still fit twice into TMEM.
+    // ... and every layer whose output is consumed (a producer) still has enough 256-row tiles to fill most of the
+    // machine WITHOUT a K-split: a split producer pays fp32 partials plus a reduce step before its consumers may start
+    // (measured: cfg 4 134.6 us with 128-row units vs 139.9 us with 256-row units; cfg 3, 112 tiles, prefers 256).
+    const int grid_guess = m.grid > 0 ? std::min(m.grid, h->num_sms) : h->num_sms;
+    bool wide_ok = h->tile_m >= 96 && h->tile_m <= 128;
+    for (int l = 0; l + 1 < h->L && wide_ok; ++l)
+        wide_ok = ceil_div(h->widths[l + 1], 2 * kTileN) * h->m_blks * 10 >= grid_guess * 7;
+    if (h->L == 1) wide_ok = wide_ok && ceil_div(h->widths[1], 2 * kTileN) * h->m_blks * 10 >= grid_guess * 7;
     if (m.tile_n == 2 * kTileN) h->n_sub = 2;
     else if (m.tile_n == kTileN) h->n_sub = 1;
-    else h->n_sub = (h->tile_m >= 96 && h->tile_m <= 128) ? 2 : 1;
+    else h->n_sub = wide_ok ? 2 : 1;
     h->acc_stages = std::max(1, std::min(kMaxAccStages, 512 / (h->n_sub * h->tile_m)));
     // Shared-memory rings: weight tiles (16 KB x n_sub each) and activation tiles (tile_m x 128 B each).
     // Weight ring depth: bytes in flight per SM just above the bandwidth-delay product (~80 KB x 148 SMs);
