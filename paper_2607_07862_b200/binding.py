@@ -40,7 +40,7 @@ class mlp_mode(ctypes.Structure):
         ("tile_m", ctypes.c_int), ("tile_n", ctypes.c_int), ("tile_k", ctypes.c_int),
         ("stages", ctypes.c_int), ("kslice_tiles", ctypes.c_int), ("split_k", ctypes.c_int),
         ("flags", ctypes.c_uint), ("split_k_layer", ctypes.c_int * MLP_MAX_LAYERS),
-        ("grid", ctypes.c_int), ("w_group", ctypes.c_int), ("timeout_ms", ctypes.c_int),
+        ("grid", ctypes.c_int), ("w_group", ctypes.c_int), ("timeout_ms", ctypes.c_int), ("a_stages", ctypes.c_int),
     ]
 
 
@@ -151,10 +151,11 @@ def _check(status: int, handle=None):
 
 def make_mode(kind: int = MLP_CTA_PIPELINED, chunks: int = 0, sm_split: float = 1.0, tile_m: int = 0, stages: int = 0,
               split_k: int = 0, split_k_layer: Sequence[int] = (), flags: int = 0, grid: int = 0,
-              timeout_ms: int = 0, w_group: int = 0, tile_n: int = 0) -> mlp_mode:
+              timeout_ms: int = 0, w_group: int = 0, tile_n: int = 0, a_stages: int = 0) -> mlp_mode:
     m = mlp_mode()
     m.kind, m.chunks, m.sm_split, m.tile_m, m.stages = kind, chunks, sm_split, tile_m, stages
     m.tile_n = tile_n
+    m.a_stages = a_stages
     m.split_k, m.flags, m.grid, m.timeout_ms = split_k, flags, grid, timeout_ms
     m.w_group = w_group
     for i, s in enumerate(split_k_layer):
