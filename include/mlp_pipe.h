@@ -106,7 +106,8 @@ enum {
                                        caller's buffers, timing each with the in-kernel clock, and keeps the
                                        fastest.  That one call synchronises the device, may allocate, and takes
                                        tens of milliseconds; Y is valid after it.  Results are remembered per
-                                       process for equal (shape, mode).  SEQUENTIAL and CTA_PIPELINED only.     */
+                                       process for equal (shape, mode).  SEQUENTIAL and CTA_PIPELINED only.  If the
+                                       first run is being captured into a CUDA graph the search is skipped for good. */
 
 typedef struct {
     int kind;        /* MLP_SEQUENTIAL | MLP_MICROBATCH | MLP_CTA_PIPELINED                           */

@@ -1155,7 +1155,11 @@ int run_impl(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStre
             if ((rc = check_ptr(h, W[l], "W[l]"))) return rc;
         cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
         if (cudaStreamIsCapturing(s, &cap) != cudaSuccess) cap = cudaStreamCaptureStatusNone;
-        if (cap == cudaStreamCaptureStatusNone) {  // no search inside a graph capture: the modelled plan runs
+        if (cap != cudaStreamCaptureStatusNone) {
+            // No search inside a graph capture -- and none later either: the captured launch holds this plan's device
+            // pointers (tables, workspace), which a later plan change would free.
+            h->tuned = true;
+        } else {
             bool cached = false;
             {
                 std::lock_guard<std::mutex> lock(g_plan_mutex);

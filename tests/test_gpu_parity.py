@@ -366,3 +366,38 @@ def test_workqueue_protocol_on_baseline_configs():
     check(inputs.Config("wq_3l", 48, (256, 1024, 512, 256), B.MLP_ACT_RELU, "exact", 9), B.make_mode(P, flags=WQ))
     err, st = sampled_rows_check(4, B.make_mode(P, flags=WQ), rows=[0, 31, 77, 127])
     assert st.n_layers == 4
+
+
+def test_autotune_flag_with_first_run_under_graph_capture():
+    """A handle created with MLP_FLAG_AUTOTUNE whose FIRST run is captured into a CUDA graph must not search then (no
+    synchronisation inside a capture) nor later (the graph holds the plan's device pointers): replays and later eager
+    runs stay exact."""
+    cfg = inputs.get_config(0, "exact")
+    X, Ws, outs, _ = oracle_outs(cfg)
+    Xd, Wd = X.cuda(), [w.cuda() for w in Ws]
+    Y = torch.zeros((cfg.M, cfg.widths[-1]), dtype=torch.bfloat16, device="cuda")
+    p = B.MlpPipe(cfg.M, cfg.widths, cfg.act, B.make_mode(P, flags=B.MLP_FLAG_AUTOTUNE))
+    warm = B.MlpPipe(cfg.M, cfg.widths, cfg.act, B.make_mode(P, split_k=3))   # encodes nothing for `p`: its first run is the captured one
+    warm.run(Xd, Wd, Y)
+    warm.close()
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            p.run(Xd, Wd, Y, stream=s)
+    for _ in range(3):
+        Y.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert np.array_equal(inputs.as_u16(Y.cpu()), outs[-1])
+    for _ in range(3):
+        Y.zero_()
+        p.run(Xd, Wd, Y)
+        torch.cuda.synchronize()
+        assert np.array_equal(inputs.as_u16(Y.cpu()), outs[-1])
+    g.replay()
+    torch.cuda.synchronize()
+    assert np.array_equal(inputs.as_u16(Y.cpu()), outs[-1])
+    assert p.stats().ready_ok == 1
+    del g
+    p.close()
