@@ -225,15 +225,19 @@ __device__ __forceinline__ void emit_cols(const uint32_t (&f)[kCols], uint32_t s
     else if (act == kActRelu) stage_cols<kCols, kActRelu>(f, buf, r);
     else stage_cols<kCols, kActNone>(f, buf, r);
     bar_sync(1, kEpiThreads);
+    // all shared-memory reads first, then all global stores: the pieces are independent, one exposed latency instead of one per piece
+    uint4 v[kCols * 16 / kEpiThreads];
 #pragma unroll
     for (int p = 0; p < kCols * 16 / kEpiThreads; ++p) {
         const int piece = p * kEpiThreads + r;  // 16 pieces of 8 features per token row
+        v[p] = ld_shared_v4(buf + static_cast<uint32_t>((piece >> 4) * kTileN + (piece & 15) * 8) * 2u);
+    }
+#pragma unroll
+    for (int p = 0; p < kCols * 16 / kEpiThreads; ++p) {
+        const int piece = p * kEpiThreads + r;
         const int j = piece >> 4, q = piece & 15;
         const int m = m_first + j, n = n_base + q * 8;
-        if (m < m_end && n < N) {
-            const uint4 v = ld_shared_v4(buf + static_cast<uint32_t>(j * kTileN + q * 8) * 2u);
-            *reinterpret_cast<uint4*>(out + static_cast<size_t>(m) * ld + n) = v;
-        }
+        if (m < m_end && n < N) *reinterpret_cast<uint4*>(out + static_cast<size_t>(m) * ld + n) = v[p];
     }
 }
 
