@@ -218,6 +218,10 @@ struct Planner {
         }
         return b;
     }
+    // a producer with large tiles whose tiles already fill most of the machine: never split in the modelled search
+    bool big_producer(int l) const {
+        return producer_in_launch(l) && reduce_mode_for(2) == kReduceUnits && h->tiles[l] * 10 >= h->grid * 7;
+    }
     int reduce_mode_for(int sp) const {
         if (sp <= 1) return kReduceNone;
         if (h->mode.flags & MLP_FLAG_WORKQUEUE) return kReduceLastArriver;  // queue entries are MMA units only
@@ -507,18 +511,34 @@ Planner make_planner(mlp_pipe* h) {
 // ones for the last layer.
 std::vector<std::vector<int>> slice_candidates(const Planner& pl, int l, bool last, int kb_floor, bool thin) {
     std::vector<std::vector<int>> cand;
+    const mlp_pipe* h = pl.h;
     const int s_max = std::max(1, std::min(64, pl.kb_total[l] / kb_floor));
-    for (int c : {1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 12, 14, 16, 20, 24, 28, 32, 40, 48, 64}) {
-        if (c > s_max || (thin && c > 20)) break;
-        if (pl.producer_in_launch(l) && c > 4 && pl.reduce_mode_for(c) == kReduceLastArriver) continue;
-        cand.push_back(pl.uniform(l, c));
+    // Priors of the MODELLED search (thin = false), from what the measured search keeps choosing on B200 -- the model
+    // ranks the finer points of a plan within +-3 us only:
+    //  * a producer with large tiles whose tiles already fill most of the machine is never split (fp32 partials + a
+    //    reduce step before its consumers may start cost more than the idle SMs);
+    //  * the last layer of a decode-sized problem gets ~12 slices tapering 6:1 (short ragged tail, two gather trips).
+    const bool big_producer = !thin && pl.big_producer(l);
+    const bool decode_last = !thin && last && !pl.force_tile_major && !pl.producer_in_launch(l) && h->tile_m <= 32 && s_max >= 12 &&
+                             h->tiles[l] * 3 <= h->grid;
+    if (big_producer) {
+        cand.push_back(pl.uniform(l, 1));
+        return cand;
     }
+    if (!decode_last)
+        for (int c : {1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 12, 14, 16, 20, 24, 28, 32, 40, 48, 64}) {
+            if (c > s_max || (thin && c > 20)) break;
+            if (pl.producer_in_launch(l) && c > 4 && pl.reduce_mode_for(c) == kReduceLastArriver) continue;
+            cand.push_back(pl.uniform(l, c));
+        }
     if (last && !pl.force_tile_major && !pl.producer_in_launch(l))
-        for (int n : {7, 10, 12, 14, 16, 20})
+        for (int n : {7, 10, 12, 14, 16, 20}) {
+            if (decode_last && (n < 10 || n > 14)) continue;
             for (double r : {3.0, 6.0}) {
                 std::vector<int> t = pl.linear_taper(l, n, r, std::max(4, kb_floor / 2));
                 if (t.size() - 1 > 4) cand.push_back(t);
             }
+        }
     return cand;
 }
 
@@ -596,6 +616,7 @@ void resolve(mlp_pipe* h) {
         if (sp <= 0) {
             sp = std::min(ceil_div(3 * h->grid, h->tiles[l]), std::max(1, pl.kb_total[l] / kb_min));
             if (pl.producer_in_launch(l) && pl.reduce_mode_for(sp) == kReduceLastArriver) sp = std::min(sp, 4);
+            if (pl.big_producer(l)) sp = 1;
         }
         h->bounds[l] = pl.uniform(l, std::min(sp, 255));
     }
