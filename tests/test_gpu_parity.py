@@ -401,3 +401,24 @@ def test_autotune_flag_with_first_run_under_graph_capture():
     assert p.stats().ready_ok == 1
     del g
     p.close()
+
+
+KNOBS = [
+    dict(grid=8), dict(grid=1, split_k=2), dict(stages=2), dict(stages=2, a_stages=2), dict(stages=3, a_stages=9), dict(w_group=2, stages=4),
+    dict(tile_n=256, tile_m=64), dict(tile_n=256, tile_m=128, split_k=3), dict(tile_n=128, tile_m=32, split_k=5),
+    dict(flags=B.MLP_FLAG_NO_W_EVICT_FIRST), dict(flags=B.MLP_FLAG_EXP_NO_PREISSUE), dict(flags=B.MLP_FLAG_EXP_NO_FAST_PATH, split_k=4),
+    dict(split_k=16), dict(split_k_layer=[1, 24]), dict(sm_split=0.9, split_k=2),
+]
+
+
+@pytest.mark.parametrize("knobs", KNOBS, ids=[str(i) for i in range(len(KNOBS))])
+@pytest.mark.parametrize("kind", [P, S])
+def test_launch_knobs_keep_results_exact(knobs, kind):
+    """Every launch-configuration knob of mlp_mode (grid size down to ONE CTA, ring depths, tile shapes, splits, hints,
+    measurement switches that keep the protocol intact) on an exact-mode problem with several M-blocks' worth of
+    tiles per layer: bits must not change, state must stay consistent."""
+    cfg = inputs.Config("knobs", 96, (512, 1536, 768), B.MLP_ACT_RELU, "exact", 21)
+    kw = dict(knobs)
+    if kind == S:
+        kw.pop("sm_split", None)
+    check(cfg, B.make_mode(kind, **kw))
