@@ -422,3 +422,31 @@ def test_launch_knobs_keep_results_exact(knobs, kind):
     if kind == S:
         kw.pop("sm_split", None)
     check(cfg, B.make_mode(kind, **kw))
+
+
+@pytest.mark.parametrize("ci,flags,runs", [(1, B.MLP_FLAG_AUTOTUNE, 1500), (1, B.MLP_FLAG_WORKQUEUE, 800), (4, 0, 400)])
+def test_soak_full_size_runs_are_bit_identical(ci, flags, runs):
+    """Full-size configs, random inputs, H poisoned every few runs: with a fixed plan the result must never change by
+    a bit from run to run (the split-K sums are taken in slice order whoever reduces; an ordering bug in the protocol
+    shows up as NaN or as a flipped bit), and the first result must be the oracle's within tolerance."""
+    cfg = inputs.CONFIGS[ci]
+    X, Ws = inputs.make_inputs(cfg)
+    Xd, Wd = X.cuda(), [w.cuda() for w in Ws]
+    p = B.MlpPipe(cfg.M, cfg.widths, cfg.act, B.make_mode(P, flags=flags))
+    Y = p.run(Xd, Wd)
+    torch.cuda.synchronize()
+    ref = Y.clone().view(torch.int16)
+    rows = [0, cfg.M // 2, cfg.M - 1]
+    outs, _ = oracle.mlp_chain(inputs.as_u16(X)[rows].copy(), [inputs.as_u16(w) for w in Ws], cfg.act)
+    e = oracle.rel_err(inputs.as_u16(Y.cpu())[rows], outs[-1])
+    assert e["nan"] == 0 and e["err"] <= TOL, e
+    bad = torch.zeros((), dtype=torch.int64, device="cuda")
+    for i in range(runs):
+        if i % 7 == 0:
+            p.poison_hidden(0x7FC0)
+        p.run(Xd, Wd, Y)
+        bad += (Y.view(torch.int16) != ref).sum()
+    assert int(bad.item()) == 0
+    st = p.stats()
+    assert st.ready_ok == 1 and st.status == 0
+    p.close()
