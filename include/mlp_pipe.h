@@ -102,7 +102,8 @@ enum {
                                        run in the order in which they became ready; the weights of a unit cannot be
                                        prefetched before the pop).  Split tiles are summed by the last-arriving slice.       */
 #define MLP_FLAG_AUTOTUNE 0x400u    /* measured plan search: the FIRST mlp_pipe_run on the handle (outside stream
-                                       capture) tries the planner's candidate K-splits / ticket orders on the
+                                       capture) tries the planner's candidate K-splits / ticket orders (and, unless tile_n is given,
+                                       both unit heights 128 / 256) on the
                                        caller's buffers, timing each with the in-kernel clock, and keeps the
                                        fastest.  That one call synchronises the device, may allocate, and takes
                                        tens of milliseconds; Y is valid after it.  Results are remembered per

@@ -953,19 +953,21 @@ int create_impl(mlp_pipe** out, int M, int L, const int* widths, int dtype, int 
 
     CREATE_TRY(cudaFuncSetAttribute(mlp_pipe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(h->smem_bytes)));
     for (int l = 0; l < L - 1; ++l) CREATE_TRY(cudaMalloc(&h->H[l], static_cast<size_t>(M) * widths[l + 1] * 2));
+    // counters are laid out for 128-row tiles (the larger count), so that the measured search may switch tile_n
     size_t words = 0;
-    for (int l = 0; l < L; ++l) words += 32 + 2 * static_cast<size_t>(round_up(h->tiles[l], 32));
+    for (int l = 0; l < L; ++l) words += 32 + 2 * static_cast<size_t>(round_up(ceil_div(widths[l + 1], kTileN) * h->m_blks, 32));
     h->counters_words = words;
     CREATE_TRY(cudaMalloc(&h->counters, words * sizeof(uint32_t)));
     {
         uint32_t* p = h->counters;
         for (int l = 0; l < L; ++l) {
+            const int t128 = round_up(ceil_div(widths[l + 1], kTileN) * h->m_blks, 32);
             h->ticket[l] = p;  // own 128-byte line
             p += 32;
             h->arrive[l] = p;
-            p += round_up(h->tiles[l], 32);
+            p += t128;
             h->ready[l] = p;
-            p += round_up(h->tiles[l], 32);
+            p += t128;
         }
     }
     CREATE_TRY(cudaMalloc(&h->epoch, kMaxLayers * sizeof(unsigned long long)));
@@ -1088,6 +1090,17 @@ int last_span_us(mlp_pipe* h, double* out) {
     return MLP_OK;
 }
 
+// Switch the handle to tile_n weight rows per unit: everything resolve() derives (rings, accumulators, tiles, modelled
+// plan) plus what depends on it outside (kernel attribute, weight tensor maps).  The caller installs the plan.
+int reshape(mlp_pipe* h, int tile_n) {
+    h->mode.tile_n = tile_n;
+    resolve(h);
+    CUDA_TRY(h, cudaFuncSetAttribute(mlp_pipe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(h->smem_bytes)));
+    for (int l = 0; l < kMaxLayers; ++l)
+        for (int i = 0; i < kTmapCache; ++i) h->cache_w[l][i].ptr = nullptr;
+    return MLP_OK;
+}
+
 // MLP_FLAG_AUTOTUNE: measured coordinate descent over the planner's slice candidates, layer by layer from the
 // last one, on the caller's buffers (every candidate computes the same Y).  Starts from the modelled plan.
 int autotune(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStream_t s) {
@@ -1097,6 +1110,7 @@ int autotune(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStre
     // search with plain stream order, run with PDL afterwards
     const std::string key = plan_key(h);
     const unsigned saved_flags = h->mode.flags;
+    const int saved_tile_n = h->mode.tile_n;
     h->mode.flags &= ~static_cast<unsigned>(MLP_FLAG_PDL);
     struct Restore {
         mlp_pipe* h;
@@ -1118,32 +1132,62 @@ int autotune(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStre
         *us = best;
         return MLP_OK;
     };
-    double best_us;
-    if ((rc = measure(&best_us))) return rc;
     const int n_launch = pl.pipelined ? 1 : h->L;
-    for (int pass = 0; pass < 2; ++pass) {
-        bool improved = false;
-        for (int l = h->L - 1; l >= 0; --l) {
-            if (h->fixed_split[l]) continue;
-            const bool last = pl.pipelined ? l == h->L - 1 : true;
-            const std::vector<int> start = h->bounds[l];
-            std::vector<int> best = start;
-            for (const auto& c : slice_candidates(pl, l, last, h->kb_floor, true)) {
-                if (c == start) continue;
-                h->bounds[l] = c;
-                pl.build_table(l, c, h->table[l], h->reduce_mode[l], h->ready_inc[l]);
-                double t;
-                if ((rc = measure(&t))) return rc;
-                if (t < best_us - 0.05 * n_launch) {
-                    best_us = t;
-                    best = c;
-                    improved = true;
+    // inner search for the current tile shape: coordinate descent over the slice candidates, layer by layer from the last
+    auto descend = [&](double* out_us) -> int {
+        double best_us;
+        int r = measure(&best_us);
+        if (r) return r;
+        for (int pass = 0; pass < 2; ++pass) {
+            bool improved = false;
+            for (int l = h->L - 1; l >= 0; --l) {
+                if (h->fixed_split[l]) continue;
+                const bool last = pl.pipelined ? l == h->L - 1 : true;
+                const std::vector<int> start = h->bounds[l];
+                std::vector<int> best = start;
+                for (const auto& c : slice_candidates(pl, l, last, h->kb_floor, true)) {
+                    if (c == start) continue;
+                    h->bounds[l] = c;
+                    pl.build_table(l, c, h->table[l], h->reduce_mode[l], h->ready_inc[l]);
+                    double t;
+                    if ((r = measure(&t))) return r;
+                    if (t < best_us - 0.05 * n_launch) {
+                        best_us = t;
+                        best = c;
+                        improved = true;
+                    }
                 }
+                h->bounds[l] = best;
+                pl.build_table(l, best, h->table[l], h->reduce_mode[l], h->ready_inc[l]);
             }
-            h->bounds[l] = best;
-            pl.build_table(l, best, h->table[l], h->reduce_mode[l], h->ready_inc[l]);
+            if (!improved) break;
         }
-        if (!improved) break;
+        *out_us = best_us;
+        return MLP_OK;
+    };
+    // outer search: weight rows per unit (128 / 256) unless the caller fixed it; starts with the heuristic's choice
+    const int tile_n_start = kTileN * h->n_sub;
+    double best_us;
+    if ((rc = descend(&best_us))) return rc;
+    int best_tile_n = tile_n_start;
+    std::vector<std::vector<int>> best_bounds(h->L);
+    for (int l = 0; l < h->L; ++l) best_bounds[l] = h->bounds[l];
+    if (saved_tile_n == 0 && h->tile_m <= 128 && h->tile_m >= 32) {
+        const int alt = tile_n_start == kTileN ? 2 * kTileN : kTileN;
+        if ((rc = reshape(h, alt))) return rc;
+        pl = make_planner(h);
+        double alt_us;
+        if ((rc = descend(&alt_us))) return rc;
+        if (alt_us < best_us - 0.2 * n_launch) {
+            best_us = alt_us;
+            best_tile_n = alt;
+            for (int l = 0; l < h->L; ++l) best_bounds[l] = h->bounds[l];
+        } else {
+            if ((rc = reshape(h, tile_n_start))) return rc;
+            pl = make_planner(h);
+        }
+        for (int l = 0; l < h->L; ++l) h->bounds[l] = best_bounds[l];
+        pl.build_all();
     }
     h->mode.flags = saved_flags;
     if ((rc = install_plan(h))) return rc;
@@ -1151,12 +1195,13 @@ int autotune(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStre
     h->tuned = true;
     {
         std::lock_guard<std::mutex> lock(g_plan_mutex);
-        std::vector<std::vector<int>> v(h->L);
+        std::vector<std::vector<int>> v(h->L + 1);
         for (int l = 0; l < h->L; ++l) v[l] = h->bounds[l];
+        v[h->L] = {best_tile_n};
         g_plan_cache[key + "#tuned"] = v;
     }
     if (getenv("MLP_PIPE_DEBUG")) {
-        fprintf(stderr, "[mlp_pipe] autotuned: %.1f us in-kernel span;", best_us);
+        fprintf(stderr, "[mlp_pipe] autotuned: %.1f us in-kernel span; tile_n %d;", best_us, best_tile_n);
         for (int l = 0; l < h->L; ++l) {
             fprintf(stderr, " L%d:", l);
             for (int b : h->bounds[l]) fprintf(stderr, " %d", b);
@@ -1182,17 +1227,21 @@ int run_impl(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStre
             h->tuned = true;
         } else {
             bool cached = false;
+            std::vector<std::vector<int>> cached_plan;
             {
                 std::lock_guard<std::mutex> lock(g_plan_mutex);
                 auto it = g_plan_cache.find(plan_key(h) + "#tuned");
                 if (it != g_plan_cache.end()) {
-                    Planner pl = make_planner(h);
-                    for (int l = 0; l < h->L; ++l) h->bounds[l] = it->second[l];
-                    pl.build_all();
+                    cached_plan = it->second;
                     cached = true;
                 }
             }
             if (cached) {
+                const int tile_n = cached_plan[h->L][0];
+                if (tile_n != kTileN * h->n_sub && (rc = reshape(h, tile_n))) return rc;
+                Planner pl = make_planner(h);
+                for (int l = 0; l < h->L; ++l) h->bounds[l] = cached_plan[l];
+                pl.build_all();
                 if ((rc = install_plan(h))) return rc;
                 h->tuned = true;
             } else if ((rc = autotune(h, X, W, Y, s))) {
