@@ -61,10 +61,14 @@ def measured_peaks():
 def committed_traffic(workload: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture, or None."""
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            return json.load(f).get(workload)
+        import csv
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == workload:
+                    return float(row["dram_bytes_per_launch"])
     except Exception:
-        return None
+        pass
+    return None
 
 
 class ClockSampler:
