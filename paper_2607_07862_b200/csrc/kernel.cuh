@@ -22,14 +22,16 @@
 //
 // Warp roles (protocol hidden in the scheduler and store warps of a
 // warp-specialised persistent kernel):
-//     warp 0  scheduler     global atomic ticket -> unit decode -> smem ring (broadcast)   [step a1]
+//     warp 0  scheduler     global atomic ticket -> unit table -> smem ring (broadcast), drawn late; fast-path look
+//                            at the unit's ready counters; in work-queue mode: pops the unit from the queue  [step a1]
 //     warp 1  W loader      TMA loads of weight tiles; never waits on a flag, so W_{l+1} is
 //                            prefetched up to the ring depth before A^l exists
-//     warp 2  A loader      consumer prologue: ld.acquire.gpu polls the (M-block, K-slice) ready
-//                            counter, then TMA-loads the activation tile                    [step a5]
+//     warp 2  A loader      consumer prologue: polls the (M-block, K-slice) ready counters (ld.relaxed.gpu + one
+//                            fence.acq_rel.gpu, or ld.acquire.gpu), then TMA-loads the activation tile [step a5]
 //     warp 3  MMA issuer    tcgen05.mma into TMEM; owns TMEM alloc / dealloc                [a2, a6]
-//     warps 4-7 epilogue    tcgen05.ld -> (split-K fix-up) -> act -> bf16 -> global store,
-//                            then producer epilogue: fence + red.release.gpu publish        [a3, a4, a7, a8]
+//     warps 4-7 epilogue    tcgen05.ld -> act -> bf16 -> transposed store, or fp32 split-K partial (+ gather by the
+//                            last arriver), or a reduce unit; then producer epilogue: fence + red.release.gpu
+//                            publish (+ scoreboard / queue push in work-queue mode)          [a3, a4, a7, a8]
 #pragma once
 #include <cuda_bf16.h>
 
