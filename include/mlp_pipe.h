@@ -101,6 +101,12 @@ enum {
                                        POSITION, the CTA spins until an entry appears there and remaps its unit to it (units
                                        run in the order in which they became ready; the weights of a unit cannot be
                                        prefetched before the pop).  Split tiles are summed by the last-arriving slice.       */
+#define MLP_FLAG_PAIR 0x2000u       /* CTA pairs (thread-block clusters of 2, tcgen05 cta_group::2):
+                                       a pair executes one unit of 256 weight rows -- each CTA stages its own 128 rows and HALF
+                                       of the activation tile, the leader schedules (one ticket per pair) and issues one MMA of
+                                       M = 256 for both tensor cores; counters, partials and outputs stay per 128-row block.
+                                       Halves the activation bytes an SM pulls per weight byte.  tile_m must be a multiple of
+                                       32 (UNSUPPORTED otherwise), grid even, not with MLP_FLAG_WORKQUEUE.                      */
 #define MLP_FLAG_AUTOTUNE 0x400u    /* measured plan search: the FIRST mlp_pipe_run on the handle (outside stream
                                        capture) tries the planner's candidate K-splits / ticket orders (and, unless tile_n is given,
                                        both unit heights 128 / 256) on the

@@ -24,6 +24,7 @@ MLP_FLAG_TILE_MAJOR, MLP_FLAG_DEBUG_DELAY, MLP_FLAG_DEBUG_REVERSE, MLP_FLAG_NO_W
 MLP_FLAG_AUTOTUNE = 0x400
 MLP_FLAG_PDL = 0x800
 MLP_FLAG_WORKQUEUE = 0x1000
+MLP_FLAG_PAIR = 0x2000
 MLP_FLAG_ACQUIRE_LOADS, MLP_FLAG_EXP_NO_ACQUIRE_FENCE, MLP_FLAG_EXP_NO_PROXY_FENCE = 0x40, 0x10, 0x20
 MLP_FLAG_EXP_NO_FAST_PATH, MLP_FLAG_EXP_NO_PREISSUE = 0x80, 0x100
 

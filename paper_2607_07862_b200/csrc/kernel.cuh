@@ -140,6 +140,8 @@ struct KernelParams {
     int w_group;        // weight K-blocks requested back to back
     int producer_ctas;  // CTAs with blockIdx.x < producer_ctas start at layer_begin, the rest one layer later
     int wait_flags;     // consumer prologue on/off
+    int pair;           // 1: CTA pairs (cluster of 2, tcgen05 cta_group::2): a pair executes one unit of 256 weight rows, each
+                        // CTA loading its 128 rows and HALF of the activation tile; the leader (rank 0) schedules and issues
     int pdl_wait;       // 1: launched as a programmatic dependent; the activation loader waits for the grid before
     uint32_t flags;
     unsigned long long* epoch_counter;  // += 1 per exiting CTA; epoch = value / gridDim.x
@@ -290,9 +292,10 @@ struct EmitCtx {
     int n_first, N, m0, m_end, act, tile_m;
 };
 
-__device__ __forceinline__ void release_acc(uint32_t bar) {
+__device__ __forceinline__ void release_acc(uint32_t bar) {  // bar & 1: pair mode, arrive on the LEADER's barrier at this offset
     tc_fence_before();
-    mbar_arrive(bar);
+    if (bar & 1u) mbar_arrive_cluster((bar & ~1u) & kPeerBitMask);
+    else mbar_arrive(bar);
 }
 
 template <int kC>
@@ -374,16 +377,35 @@ __device__ __forceinline__ void poll_counter(const uint32_t* ctr, uint32_t targe
     fence_acq_rel_gpu();
 }
 
+// arrive on the barrier at this offset in the pair LEADER's shared memory (own barrier when not in pair mode)
+__device__ __forceinline__ void arrive_leader(uint32_t bar, bool pair) {
+    if (pair) mbar_arrive_cluster(bar & kPeerBitMask);
+    else mbar_arrive(bar);
+}
+// wait on an own barrier that the other CTA of the pair may arrive on (acquire at cluster scope then)
+__device__ __forceinline__ void wait_shared(uint32_t bar, uint32_t parity, bool pair) {
+    if (pair) mbar_wait_cluster(bar, parity);
+    else mbar_wait(bar, parity);
+}
+
+// kPair: the CTA-pair build (tcgen05 cta_group::2).  A separate instantiation because a kernel that contains cta_group::2
+// instructions can only be launched in clusters of two.
+template <bool kPair>
 __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_constant__ KernelParams P) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
 
     const int tile_m = P.tile_m;
+    constexpr bool pair = kPair;
+    const uint32_t rank = pair ? cluster_ctarank() : 0u;   // rank in the CTA pair; the leader is rank 0
+    const bool leader = rank == 0;
+    const int nb_mul = pair ? 2 : 1;                       // 128-row counter tiles per table tile
+    const int a_rows = pair ? tile_m / 2 : tile_m;         // token rows of the activation tile this CTA stages
     const int n_sub = P.n_sub;
     const int tile_n = kTileN * n_sub;  // weight rows per unit
     const uint32_t w_tile_bytes = static_cast<uint32_t>(n_sub) * kWTileBytes;
-    const uint32_t a_tile_bytes = static_cast<uint32_t>(tile_m) * (kTileK * 2);
+    const uint32_t a_tile_bytes = static_cast<uint32_t>(a_rows) * (kTileK * 2);
     const int stages = P.stages;      // weight ring depth
     const int a_stages = P.a_stages;  // activation ring depth (its own, deeper ring: the consumer prologue's
                                       // polls and fences then run K-blocks ahead of the weight stream)
@@ -440,9 +462,9 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
         constexpr int kNumBars = 4 * kMaxStages + 2 * kMaxAccStages + 3 * kSchedSlots;
         for (int b = lane; b < kNumBars; b += 32) {
             uint32_t count = 1;
-            if (b >= 4 * kMaxStages + kMaxAccStages && b < 4 * kMaxStages + 2 * kMaxAccStages) count = kEpiThreads;                   // tempty
+            if (b >= 4 * kMaxStages + kMaxAccStages && b < 4 * kMaxStages + 2 * kMaxAccStages) count = kEpiThreads * nb_mul;          // tempty (pair: both CTAs' epilogues)
             if (b >= 4 * kMaxStages + 2 * kMaxAccStages + kSchedSlots && b < 4 * kMaxStages + 2 * kMaxAccStages + 2 * kSchedSlots)
-                count = 3 + kEpiThreads;                                                                                              // sempty
+                count = (3 + kEpiThreads) * nb_mul;                                                                                   // sempty (pair: both CTAs' consumers)
             mbar_init(bar_full + 8 * b, count);
         }
         fence_mbar_init();
@@ -460,7 +482,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
             l0 = P.layer_begin + 1;
             sid = blockIdx.x - P.producer_ctas;
         }
-        const bool have = sid < static_cast<uint32_t>(P.layer[l0].units) &&
+        const bool have = !pair && sid < static_cast<uint32_t>(P.layer[l0].units) &&
                           !(P.layer[l0].use_queue && P.wait_flags && l0 > P.layer_begin);  // (a queue-mode unit is unknown until popped)
         uint2 raw = make_uint2(0u, 0u);
         prefetch_tmap(&P.tm_w[l0]);
@@ -512,11 +534,17 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
         }
     }
     if (warp == 3) {
-        tmem_alloc(smem_u32(const_cast<uint32_t*>(s_tmem)), tmem_cols);
-        tmem_relinquish();
+        if (pair) {  // the same warp of both CTAs allocates the same columns in both TMEMs
+            tmem_alloc_pair(smem_u32(const_cast<uint32_t*>(s_tmem)), tmem_cols);
+            tmem_relinquish_pair();
+        } else {
+            tmem_alloc(smem_u32(const_cast<uint32_t*>(s_tmem)), tmem_cols);
+            tmem_relinquish();
+        }
     }
     tc_fence_before();
-    __syncthreads();
+    if (pair) cluster_sync_all();  // the peer's barriers are initialised before anything arrives on them remotely
+    else __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *s_tmem;
     const unsigned long long epoch = *s_epoch;
@@ -524,19 +552,20 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
 
     // ------------------------------------------------------------------ roles
     if (warp == 0) {
-        // ===== scheduler: ticket -> unit (step a1, ordering knob PAPER.md:99-101)
-        if (lane == 0) {
+        // ===== scheduler: ticket -> unit (step a1, ordering knob PAPER.md:99-101); in pair mode only
+        // the leader CTA schedules and hands every unit to both CTAs' rings
+        if (lane == 0 && leader) {
             uint32_t done[kMaxLayers];
             for (int l = 0; l < kMaxLayers; ++l) done[l] = 0;
             unsigned long long q_stall = 0, q_polls = 0;
             int l = P.layer_begin;
             // the first unit of a CTA is static (its rank among the CTAs that start on the same layer):
             // no atomic round trip before the first weight load
-            uint32_t static_id = blockIdx.x;
+            uint32_t static_id = blockIdx.x / nb_mul;  // worker index (a worker = a CTA, or a CTA pair)
             bool use_static = true;
-            if (static_cast<int>(blockIdx.x) >= P.producer_ctas && P.layer_begin + 1 < P.layer_end) {
+            if (static_cast<int>(static_id) >= P.producer_ctas && P.layer_begin + 1 < P.layer_end) {
                 l = P.layer_begin + 1;
-                static_id = blockIdx.x - P.producer_ctas;
+                static_id -= P.producer_ctas;
             }
             uint32_t it = 0;
             bool finished = false;
@@ -613,6 +642,8 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                     u.valid = 1;
                     if (popped) {
                         u.acquired = 1;
+                    } else if (u.kind == kUnitReduce && pair) {
+                        // each CTA of the pair reduces its own 128 rows and polls its own arrival counter
                     } else if (u.kind == kUnitReduce) {
                         // fast path of a reduce unit: all slices of its tile have already arrived
                         const uint32_t target = static_cast<uint32_t>((epoch + 1ull) * static_cast<unsigned long long>(L.split));
@@ -620,7 +651,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                             fence_acq_rel_gpu();
                             u.acquired = 1;
                         }
-                    } else if (P.wait_flags && l > P.layer_begin && !(P.flags & (kFlagExpNoFastPath | kFlagAcquireLoads))) {
+                    } else if (P.wait_flags && l > P.layer_begin && !pair && !(P.flags & (kFlagExpNoFastPath | kFlagAcquireLoads))) {
                         // Consumer prologue, fast path (the prologue lives in the scheduler
                         // warp): one look at all ready counters under this unit's K range.  If every producer
                         // tile is already published -- the normal case, the scheduler runs a unit ahead --
@@ -649,9 +680,18 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 }
                 finished = !u.valid;
                 const uint32_t slot = it % kSchedSlots;
-                if (it >= kSchedSlots) mbar_wait(bar_sempty + 8 * slot, ((it / kSchedSlots) & 1) ^ 1);
+                if (it >= kSchedSlots) wait_shared(bar_sempty + 8 * slot, ((it / kSchedSlots) & 1) ^ 1, pair);
                 ring[slot] = u;
-                mbar_arrive(bar_sfull + 8 * slot);  // release: ring[slot] visible to waiters
+                if (pair) {  // the same slot of the peer's ring, then both "slot full" barriers (release at cluster scope)
+                    const uint32_t peer_slot = mapa_u32(smem_u32(&ring[slot]), 1u);
+                    const uint32_t* w = reinterpret_cast<const uint32_t*>(&u);
+#pragma unroll
+                    for (int i = 0; i < static_cast<int>(sizeof(UnitInfo) / 4); ++i) st_cluster_u32(peer_slot + 4 * i, w[i]);
+                    mbar_arrive_cluster(mapa_u32(bar_sfull + 8 * slot, 1u));
+                    mbar_arrive_cluster(bar_sfull + 8 * slot);
+                } else {
+                    mbar_arrive(bar_sfull + 8 * slot);  // release: ring[slot] visible to waiters
+                }
                 ++it;
             }
             for (int l2 = 0; l2 < kMaxLayers; ++l2) P.stats[blockIdx.x].units[l2] = done[l2];
@@ -669,9 +709,9 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
             unsigned long long w_wait = 0;
             for (uint32_t it = 0;; ++it) {
                 const uint32_t slot = it % kSchedSlots;
-                mbar_wait(bar_sfull + 8 * slot, (it / kSchedSlots) & 1);
+                wait_shared(bar_sfull + 8 * slot, (it / kSchedSlots) & 1, pair);
                 const UnitInfo u = ring[slot];
-                mbar_arrive(bar_sempty + 8 * slot);
+                arrive_leader(bar_sempty + 8 * slot, pair);
                 // Late binding: the scheduler may draw the NEXT ticket only once this unit has at most
                 // claim_ahead K-blocks left to request.  A unit stalled on its producers (the ring is full, the
                 // MMA warp waits for the activation loader) therefore never holds a second ticket.
@@ -712,10 +752,16 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                     }
                     for (int i = 0; i < g; ++i, ++kb) {
                         const uint32_t full = bar_full + 8 * stage;
-                        mbar_arrive_expect_tx(full, w_tile_bytes);
                         const uint32_t dst = smem_base + stage * w_tile_bytes;
-                        if (hint) tma_load_2d_hint(dst, tm, kb * kTileK, u.n_blk * tile_n, full, pol);
-                        else tma_load_2d(dst, tm, kb * kTileK, u.n_blk * tile_n, full);
+                        if (pair) {
+                            // each CTA loads its own 128 weight rows; the bytes of BOTH count on the leader's barrier
+                            if (leader) mbar_arrive_expect_tx(full, 2 * w_tile_bytes);
+                            tma_load_2d_pair(dst, tm, kb * kTileK, (u.n_blk * 2 + static_cast<int>(rank)) * kTileN, full, pol);
+                        } else {
+                            mbar_arrive_expect_tx(full, w_tile_bytes);
+                            if (hint) tma_load_2d_hint(dst, tm, kb * kTileK, u.n_blk * tile_n, full, pol);
+                            else tma_load_2d(dst, tm, kb * kTileK, u.n_blk * tile_n, full);
+                        }
                         if (++stage == static_cast<uint32_t>(stages)) { stage = 0; phase ^= 1; }
                     }
                 }
@@ -729,6 +775,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
             uint32_t stage = 0, phase = 0;
             unsigned long long stall = 0, polls = 0;
             bool aborted = false;
+            const uint64_t pol_a = policy_evict_normal();
             if (P.pdl_wait) {
                 // programmatic dependent launch (stronger SEQUENTIAL baseline): this grid was allowed to start while
                 // the grid of the layer before still runs; setup and the weight prefetch overlap its tail, and only
@@ -738,9 +785,9 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
             }
             for (uint32_t it = 0;; ++it) {
                 const uint32_t slot = it % kSchedSlots;
-                mbar_wait(bar_sfull + 8 * slot, (it / kSchedSlots) & 1);
+                wait_shared(bar_sfull + 8 * slot, (it / kSchedSlots) & 1, pair);
                 const UnitInfo u = ring[slot];
-                mbar_arrive(bar_sempty + 8 * slot);
+                arrive_leader(bar_sempty + 8 * slot, pair);
                 if (!u.valid) break;
                 if (u.kind == kUnitReduce) continue;
                 const CUtensorMap* tm = &P.tm_a[u.layer];
@@ -748,7 +795,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 if (P.wait_flags && u.layer > P.layer_begin) fence_proxy_async();
                 const LayerParams& Lp = P.layer[u.layer > 0 ? u.layer - 1 : 0];
                 const uint32_t target = static_cast<uint32_t>((epoch + 1ull) * static_cast<unsigned long long>(Lp.ready_inc));
-                const uint32_t* ready = wait ? Lp.ready + u.m_blk * Lp.n_blks : nullptr;
+                const uint32_t* ready = wait ? Lp.ready + u.m_blk * Lp.n_blks * nb_mul : nullptr;
                 // Slices [.., ready_upto) of this unit are known to be published.  Readiness is monotone
                 // within a run, so the prologue looks ahead: up to 8 counters are read with independent
                 // relaxed loads that are ISSUED a few K-blocks before their result is needed (the round trip
@@ -810,8 +857,14 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                             pend_base = -1;
                         }
                     }
-                    mbar_arrive_expect_tx(bar_afull + 8 * stage, a_tile_bytes);
-                    tma_load_2d(a_ring + stage * a_tile_bytes, tm, kb * kTileK, P.m_off + u.m_blk * tile_m, bar_afull + 8 * stage);
+                    if (pair) {  // each CTA stages HALF of the tokens (the B operand of the pair MMA is split between the CTAs)
+                        if (leader) mbar_arrive_expect_tx(bar_afull + 8 * stage, 2 * a_tile_bytes);
+                        tma_load_2d_pair(a_ring + stage * a_tile_bytes, tm, kb * kTileK, P.m_off + u.m_blk * tile_m + static_cast<int>(rank) * a_rows,
+                                         bar_afull + 8 * stage, pol_a);
+                    } else {
+                        mbar_arrive_expect_tx(bar_afull + 8 * stage, a_tile_bytes);
+                        tma_load_2d(a_ring + stage * a_tile_bytes, tm, kb * kTileK, P.m_off + u.m_blk * tile_m, bar_afull + 8 * stage);
+                    }
                     if (++stage == static_cast<uint32_t>(a_stages)) { stage = 0; phase ^= 1; }
                 }
             }
@@ -823,19 +876,22 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
     } else if (warp == 3) {
         // ===== MMA issuer (steps a2, a6)
         if (lane == 0) {
-            const uint32_t idesc = make_idesc_bf16(kTileN, tile_m);
+            // pair mode: ONE instruction of the leader drives both tensor cores -- M = 256 (128 weight rows per CTA), the
+            // tile_m tokens of the B operand half in each CTA's shared memory, D in both TMEMs at the same address
+            const uint32_t idesc = make_idesc_bf16(pair ? 2 * kTileN : kTileN, tile_m);
             uint32_t stage = 0, phase = 0, astage = 0, aphase = 0;
             unsigned long long wait_ops = 0, wait_acc = 0;
             uint32_t mma_it = 0;  // MMA units so far: picks the accumulator (the epilogue warps count alike)
             for (uint32_t it = 0;; ++it) {
                 const uint32_t slot = it % kSchedSlots;
-                mbar_wait(bar_sfull + 8 * slot, (it / kSchedSlots) & 1);
+                wait_shared(bar_sfull + 8 * slot, (it / kSchedSlots) & 1, pair);
                 const UnitInfo u = ring[slot];
-                mbar_arrive(bar_sempty + 8 * slot);
+                arrive_leader(bar_sempty + 8 * slot, pair);
                 if (!u.valid) break;
-                if (u.kind == kUnitReduce) continue;
+                if (u.kind == kUnitReduce || !leader) continue;  // (the peer's MMA warp only keeps its ring in step)
                 const uint32_t acc = mma_it % acc_stages;
-                mbar_wait_timed(bar_tempty + 8 * acc, ((mma_it / acc_stages) & 1u) ^ 1u, wait_acc);
+                if (pair) wait_shared(bar_tempty + 8 * acc, ((mma_it / acc_stages) & 1u) ^ 1u, true);
+                else mbar_wait_timed(bar_tempty + 8 * acc, ((mma_it / acc_stages) & 1u) ^ 1u, wait_acc);
                 ++mma_it;
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + acc * acc_cols;
@@ -855,15 +911,22 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                         for (int k = 0; k < kTileK / kUmmaK; ++k) {
                             // advancing K by 16 bf16 = 32 B inside the 128 B swizzle span: +2 in the
                             // (addr >> 4) field of the descriptor
-                            umma_bf16(d_tmem + rr * tile_m, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb > u.kb0 || k > 0) ? 1u : 0u);
+                            if (pair) umma_bf16_pair(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb > u.kb0 || k > 0) ? 1u : 0u);
+                            else umma_bf16(d_tmem + rr * tile_m, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb > u.kb0 || k > 0) ? 1u : 0u);
                         }
                     }
-                    umma_commit(bar_empty + 8 * stage);
-                    umma_commit(bar_aempty + 8 * astage);
+                    if (pair) {  // the stages of BOTH CTAs are free again
+                        umma_commit_pair(bar_empty + 8 * stage);
+                        umma_commit_pair(bar_aempty + 8 * astage);
+                    } else {
+                        umma_commit(bar_empty + 8 * stage);
+                        umma_commit(bar_aempty + 8 * astage);
+                    }
                     if (++stage == static_cast<uint32_t>(stages)) { stage = 0; phase ^= 1; }
                     if (++astage == static_cast<uint32_t>(a_stages)) { astage = 0; aphase ^= 1; }
                 }
-                umma_commit(bar_tfull + 8 * acc);
+                if (pair) umma_commit_pair(bar_tfull + 8 * acc);  // both CTAs' epilogues drain their own 128 lanes
+                else umma_commit(bar_tfull + 8 * acc);
             }
             my_stats->wait[2] = wait_ops;
             my_stats->wait[3] = wait_acc;
@@ -876,16 +939,20 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
         uint32_t mma_it = 0, parity = 0;
         for (uint32_t it = 0;; ++it) {
             const uint32_t slot = it % kSchedSlots;
-            mbar_wait(bar_sfull + 8 * slot, (it / kSchedSlots) & 1);
+            wait_shared(bar_sfull + 8 * slot, (it / kSchedSlots) & 1, pair);
             const UnitInfo u = ring[slot];
-            mbar_arrive(bar_sempty + 8 * slot);
+            arrive_leader(bar_sempty + 8 * slot, pair);
             if (!u.valid) break;
             const LayerParams& L = P.layer[u.layer];
             const int m0 = P.m_off + u.m_blk * tile_m;
             const size_t out_row = static_cast<size_t>(L.N);
             const size_t blk_stride = static_cast<size_t>(tile_m) * kTileN;        // floats per 128-row block of a partial
             const size_t ks_stride = blk_stride * n_sub;                           // floats per slice
-            float* const ws_tile = L.ws + static_cast<size_t>(u.tile) * L.split * ks_stride;
+            // this CTA's 128-row block of the unit: in pair mode the CTAs of a pair own adjacent blocks, and every counter,
+            // partial and output column is indexed per 128-row block exactly as without pairing
+            const int nblk_c = u.n_blk * nb_mul + static_cast<int>(rank);
+            const int ctile = u.m_blk * (L.n_blks * nb_mul) + nblk_c;
+            float* const ws_tile = L.ws + static_cast<size_t>(ctile) * L.split * ks_stride;
             bool stored = false;  // this unit wrote (part of) the layer's output
             int red_c0 = 0, red_c1 = 0;  // token columns of the tile whose partials this unit sums (none if equal)
             if (u.kind == kUnitReduce) {
@@ -893,7 +960,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 if (it < kUnitTrace && r == 0) my_stats->unit_ts[it][2] = globaltimer_ns();
                 if (!u.acquired) {
                     if (r == 0)
-                        poll_counter(L.arrive + u.tile, static_cast<uint32_t>((epoch + 1ull) * static_cast<unsigned long long>(L.split)),
+                        poll_counter(L.arrive + ctile, static_cast<uint32_t>((epoch + 1ull) * static_cast<unsigned long long>(L.split)),
                                      P.status, P.timeout_ns, wait_part);
                     bar_sync(1, kEpiThreads);  // thread 0's acquire happens-before everybody's loads below
                 }
@@ -910,8 +977,8 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 if (it < kUnitTrace && r == 0) my_stats->unit_ts[it][2] = globaltimer_ns();
                 const long long te0 = clock64();
                 if (L.split == 1) {
-                    const EmitCtx e{stage_s, r, L.out, out_row, u.n_blk * tile_n, L.N, m0, P.m_end, L.act, tile_m};
-                    drain_acc<16, true>(taddr, static_cast<int>(acc_cols), bar_tempty + 8 * acc, e, parity, nullptr);
+                    const EmitCtx e{stage_s, r, L.out, out_row, nblk_c * tile_n, L.N, m0, P.m_end, L.act, tile_m};
+                    drain_acc<16, true>(taddr, static_cast<int>(acc_cols), (bar_tempty + 8 * acc) | (pair ? 1u : 0u), e, parity, nullptr);
                     stored = true;
                     t_direct += static_cast<unsigned long long>(clock64() - te0);
                 } else {
@@ -920,7 +987,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                     // (the columns of the n_sub blocks are consecutive both in TMEM and in the partial)
                     float* wsp = ws_tile + static_cast<size_t>(u.ks) * ks_stride + static_cast<size_t>(r) * 4;
                     const EmitCtx e{};
-                    drain_acc<16, false>(taddr, static_cast<int>(acc_cols), bar_tempty + 8 * acc, e, parity, wsp);
+                    drain_acc<16, false>(taddr, static_cast<int>(acc_cols), (bar_tempty + 8 * acc) | (pair ? 1u : 0u), e, parity, wsp);
                     // the 128 threads' partial stores happen-before thread 0's atomic (bar.sync); its release half
                     // is cumulative and publishes the CTA's whole partial, its acquire half (on the last arrival)
                     // makes the other slices' partials visible to the loads after the second barrier
@@ -931,7 +998,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                         // Nobody ever waits, so a slow slice delays only its own tile.
                         if (r == 0) {
                             const uint32_t base = static_cast<uint32_t>(epoch * static_cast<unsigned long long>(L.split));
-                            const uint32_t old = atom_add_acq_rel_gpu(L.arrive + u.tile, 1u) - base;
+                            const uint32_t old = atom_add_acq_rel_gpu(L.arrive + ctile, 1u) - base;
                             *s_last = (old == static_cast<uint32_t>(L.split - 1)) ? 1u : 0u;
                         }
                         bar_sync(1, kEpiThreads);
@@ -940,7 +1007,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                         if (last) red_c1 = tile_m;
                     } else {
                         // reduce units (their own tickets, later in this layer's table) finish the tile
-                        if (r == 0) red_release_gpu_add(L.arrive + u.tile, 1u);
+                        if (r == 0) red_release_gpu_add(L.arrive + ctile, 1u);
                     }
                 }
             }
@@ -948,7 +1015,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 const long long tg0 = clock64();
                 for (int rr = 0; rr < n_sub; ++rr) {
                     const float* blk = ws_tile + rr * blk_stride;
-                    const int n_base = u.n_blk * tile_n + rr * kTileN;
+                    const int n_base = nblk_c * tile_n + rr * kTileN;
                     for (int c = red_c0; c < red_c1; c += 16) {
                         float f[16];
                         uint32_t w[16];
@@ -973,7 +1040,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                     __nanosleep((hsh & 1023u) * 16u);
                 }
                 bar_sync(1, kEpiThreads);
-                if (r == 0) red_release_gpu_add(L.ready + u.tile, 1u);  // release: orders the tile before the counter
+                if (r == 0) red_release_gpu_add(L.ready + ctile, 1u);  // release: orders the tile before the counter
                 if (r == 0 && P.wait_flags && u.layer + 1 < P.layer_end && P.layer[u.layer + 1].use_queue) {
                     // Producer epilogue of the paper's protocol (PAPER.md:95 steps (2)-(4)): look the tile up in the
                     // dependency array, update the scoreboard entry of every group that depends on it, and push the
@@ -1008,10 +1075,12 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
 
     // ------------------------------------------------------------------ teardown
     tc_fence_before();
-    __syncthreads();
+    if (pair) cluster_sync_all();  // neither CTA leaves (or frees TMEM) while the other may still touch its shared memory / TMEM
+    else __syncthreads();
     if (warp == 3) {
         tc_fence_after();
-        tmem_dealloc(tmem_base, tmem_cols);
+        if (pair) tmem_dealloc_pair(tmem_base, tmem_cols);
+        else tmem_dealloc(tmem_base, tmem_cols);
     }
     if (threadIdx.x == 0) {
         my_stats->cycles = static_cast<unsigned long long>(clock64() - t_start);

@@ -47,6 +47,8 @@ struct mlp_pipe {
     int rows_per_launch = 0;  // M, or M / chunks
     int tile_m = 0, m_blks = 0, n_sub = 1, stages = 0, a_stages = 0, acc_stages = 0, grid = 0, producer_ctas = 0;
     size_t smem_bytes = 0;
+    int pair = 0;      // MLP_FLAG_PAIR: CTA pairs; a WORKER (who draws tickets) is then a pair
+    int workers = 0;   // grid, or grid / 2
     int split[kMaxLayers] = {0};
     int reduce_mode[kMaxLayers] = {0};
     int ready_inc[kMaxLayers] = {0};
@@ -155,6 +157,8 @@ int validate_mode(const mlp_mode& m, int M) {
     if (m.kind == MLP_MICROBATCH && (m.chunks < 1 || M % m.chunks != 0)) return MLP_ERR_INVALID;
     if (m.sm_split < 0.0f || m.sm_split > 1.0f) return MLP_ERR_INVALID;
     if (m.tile_m < 0 || m.tile_m % 16 != 0) return MLP_ERR_INVALID;
+    if ((m.flags & MLP_FLAG_PAIR) && ((m.flags & MLP_FLAG_WORKQUEUE) || m.tile_n == 2 * kTileN || (m.tile_m % 32) != 0 || (m.grid & 1)))
+        return MLP_ERR_UNSUPPORTED;
     if (m.stages < 0 || m.split_k < 0 || m.grid < 0 || m.timeout_ms < 0 || m.w_group < 0 || m.a_stages < 0) return MLP_ERR_INVALID;
     for (int l = 0; l < kMaxLayers; ++l)
         if (m.split_k_layer[l] < 0) return MLP_ERR_INVALID;
@@ -191,7 +195,7 @@ struct Planner {
 
     bool producer_in_launch(int l) const { return pipelined && l < h->L - 1; }
     bool consumer_in_launch(int l) const { return pipelined && l > 0; }
-    size_t partial_bytes() const { return static_cast<size_t>(h->n_sub) * h->tile_m * kTileN * 4; }
+    size_t partial_bytes() const { return static_cast<size_t>(h->pair ? 2 : h->n_sub) * h->tile_m * kTileN * 4; }
 
     std::vector<int> uniform(int l, int sp) const {
         sp = std::max(1, std::min(sp, kb_total[l]));
@@ -220,7 +224,7 @@ struct Planner {
     }
     // a producer with large tiles whose tiles already fill most of the machine: never split in the modelled search
     bool big_producer(int l) const {
-        return producer_in_launch(l) && reduce_mode_for(2) == kReduceUnits && h->tiles[l] * 10 >= h->grid * 7;
+        return producer_in_launch(l) && reduce_mode_for(2) == kReduceUnits && h->tiles[l] * 10 >= h->workers * 7;
     }
     int reduce_mode_for(int sp) const {
         if (sp <= 1) return kReduceNone;
@@ -232,7 +236,7 @@ struct Planner {
     }
     // token columns per reduce unit: about one reduce unit per CTA and layer, at least 16 columns
     int reduce_cols(int l) const {
-        const int chunks = std::max(1, std::min(h->tile_m / 16, (h->grid + h->tiles[l] - 1) / h->tiles[l]));
+        const int chunks = std::max(1, std::min(h->tile_m / 16, (h->workers + h->tiles[l] - 1) / h->tiles[l]));
         return ((h->tile_m + chunks - 1) / chunks + 15) / 16 * 16;
     }
 
@@ -290,7 +294,7 @@ struct Planner {
         }
         // tile-major: interleave.  Tile t's last slice has ticket (t + 1) sp - 1; its reduce units go after
         // ticket (t + 1) sp - 1 + delay of the MMA sequence.
-        const int delay = h->grid + h->grid / 4;
+        const int delay = h->workers + h->workers / 4;
         std::vector<UnitDesc> merged;
         merged.reserve(out.size() + static_cast<size_t>(tiles) * chunks);
         int next_red = 0;
@@ -315,7 +319,7 @@ struct Planner {
     // and the workers that are streaming weights at the same moment SHARE the HBM bandwidth (a worker alone is
     // limited by its own ring / L2 port / tensor core instead).  Returns the time the last output is stored.
     double makespan(int lb, int le, double cutoff = 1e30) const {
-        const int G = h->grid, R = h->n_sub, tm = h->tile_m;
+        const int G = h->workers, R = h->pair ? 2 : h->n_sub, tm = h->tile_m;
         const double w_bytes = R * static_cast<double>(kWTileBytes), a_bytes = tm * 128.0;
         // per K-block and worker: floor set by the worker's own limits ...
         const double t_cap = std::max({kDramLatencyUs / h->stages, (w_bytes + a_bytes) / kSmBytesPerUs,
@@ -520,7 +524,7 @@ std::vector<std::vector<int>> slice_candidates(const Planner& pl, int l, bool la
     //  * the last layer of a decode-sized problem gets ~12 slices tapering 6:1 (short ragged tail, two gather trips).
     const bool big_producer = !thin && pl.big_producer(l);
     const bool decode_last = !thin && last && !pl.force_tile_major && !pl.producer_in_launch(l) && h->tile_m <= 32 && s_max >= 12 &&
-                             h->tiles[l] * 3 <= h->grid;
+                             h->tiles[l] * 3 <= h->workers;
     if (big_producer) {
         cand.push_back(pl.uniform(l, 1));
         return cand;
@@ -565,6 +569,10 @@ void resolve(mlp_pipe* h) {
     if (m.tile_n == 2 * kTileN) h->n_sub = 2;
     else if (m.tile_n == kTileN) h->n_sub = 1;
     else h->n_sub = wide_ok ? 2 : 1;
+    // CTA pairs (MLP_FLAG_PAIR): a pair's unit is 256 weight rows x tile_m tokens, each CTA stages its own 128 rows and
+    // HALF of the activation tile, and keeps a 128-row accumulator of tile_m columns -- n_sub = 1 per CTA
+    h->pair = (m.flags & MLP_FLAG_PAIR) ? 1 : 0;
+    if (h->pair) h->n_sub = 1;
     h->acc_stages = std::max(1, std::min(kMaxAccStages, 512 / (h->n_sub * h->tile_m)));
     // Shared-memory rings: weight tiles (16 KB x n_sub each) and activation tiles (tile_m x 128 B each).
     // Weight ring depth: bytes in flight per SM just above the bandwidth-delay product (~80 KB x 148 SMs);
@@ -572,7 +580,7 @@ void resolve(mlp_pipe* h) {
     // Activation ring: deeper (its tiles are small at decode batch sizes), so that the consumer prologue's
     // polls and fences run well ahead of the weight stream.
     const int w_tile = h->n_sub * kWTileBytes;
-    const int a_tile = h->tile_m * kTileK * 2;
+    const int a_tile = (h->pair ? h->tile_m / 2 : h->tile_m) * kTileK * 2;
     const int max_smem = 227 * 1024 - kCtrlBytes - 1024 - kStageBytes;
     // (Measured on cfg 2, 16 KB weight + 32 KB activation tiles: 4 + 4 stages 82.4 us, 5 + 3 84.5, 6 + 3 86.5, 5 + 2 98.9 --
     // the activation ring needs its depth although it is fed from L2; mode.a_stages overrides.)
@@ -589,10 +597,12 @@ void resolve(mlp_pipe* h) {
     h->a_stages = ast;
     h->smem_bytes = static_cast<size_t>(st) * w_tile + static_cast<size_t>(ast) * a_tile + kStageBytes + kCtrlBytes + 1024;
     h->grid = m.grid > 0 ? std::min(m.grid, h->num_sms) : h->num_sms;
+    if (h->pair) h->grid &= ~1;
+    h->workers = h->pair ? h->grid / 2 : h->grid;
     const float s = (m.sm_split <= 0.0f) ? 1.0f : m.sm_split;
-    h->producer_ctas = h->grid;
+    h->producer_ctas = h->workers;  // (counted in workers)
     if (m.kind == MLP_CTA_PIPELINED && h->L > 1 && s < 1.0f)
-        h->producer_ctas = std::min(h->grid, std::max(1, static_cast<int>(h->grid * s + 0.5f)));
+        h->producer_ctas = std::min(h->workers, std::max(1, static_cast<int>(h->workers * s + 0.5f)));
 
     Planner pl;
     pl.h = h;
@@ -600,7 +610,7 @@ void resolve(mlp_pipe* h) {
     pl.force_tile_major = (m.flags & (MLP_FLAG_TILE_MAJOR | MLP_FLAG_DEBUG_REVERSE)) != 0;
     for (int l = 0; l < h->L; ++l) {
         pl.kb_total[l] = ceil_div(h->widths[l], kTileK);
-        h->tiles[l] = ceil_div(h->widths[l + 1], kTileN * h->n_sub) * h->m_blks;
+        h->tiles[l] = ceil_div(h->widths[l + 1], kTileN * (h->pair ? 2 : h->n_sub)) * h->m_blks;
     }
     // smallest slice worth a unit: the fp32 partial of a split tile should stay below ~1/8 of the operand
     // bytes the slice streams
@@ -614,7 +624,7 @@ void resolve(mlp_pipe* h) {
         fixed[l] = sp > 0;
         h->fixed_split[l] = fixed[l];
         if (sp <= 0) {
-            sp = std::min(ceil_div(3 * h->grid, h->tiles[l]), std::max(1, pl.kb_total[l] / kb_min));
+            sp = std::min(ceil_div(3 * h->workers, h->tiles[l]), std::max(1, pl.kb_total[l] / kb_min));
             if (pl.producer_in_launch(l) && pl.reduce_mode_for(sp) == kReduceLastArriver) sp = std::min(sp, 4);
             if (pl.big_producer(l)) sp = 1;
         }
@@ -704,14 +714,14 @@ int build_base_params(mlp_pipe* h) {
         Lp.K = h->widths[l];
         Lp.N = h->widths[l + 1];
         Lp.kb_total = ceil_div(Lp.K, kTileK);
-        Lp.n_blks = ceil_div(Lp.N, kTileN * h->n_sub);
+        Lp.n_blks = ceil_div(Lp.N, kTileN * (h->pair ? 2 : h->n_sub));  // table tiles per M-block (pair mode: pairs of 128-row blocks)
         Lp.split = h->split[l];
         Lp.units = static_cast<int>(h->table[l].size());
         Lp.act = l < h->L - 1 ? h->act : kActNone;
         Lp.publish = l < h->L - 1 ? 1 : 0;
         Lp.reduce_mode = h->reduce_mode[l];
         {   // do the first `grid` tickets follow the closed form (tile-major, equal slices)?
-            const int sp = h->split[l], n = std::min<int>(h->grid, static_cast<int>(h->table[l].size()));
+            const int sp = h->split[l], n = std::min<int>(h->workers, static_cast<int>(h->table[l].size()));
             bool ok = sp <= 255;
             for (int t = 0; t < n && ok; ++t) {
                 const UnitDesc& d = h->table[l][t];
@@ -742,7 +752,7 @@ int build_base_params(mlp_pipe* h) {
         Lp.arrive = h->arrive[l];
         Lp.ready = h->ready[l];
         if (l > 0) {
-            int rc = encode_2d(h, &P.tm_a[l], h->H[l - 1], h->M, h->widths[l], h->tile_m);
+            int rc = encode_2d(h, &P.tm_a[l], h->H[l - 1], h->M, h->widths[l], h->pair ? h->tile_m / 2 : h->tile_m);
             if (rc) return rc;
         }
     }
@@ -751,6 +761,7 @@ int build_base_params(mlp_pipe* h) {
     P.stages = h->stages;
     P.a_stages = h->a_stages;
     P.n_sub = h->n_sub;
+    P.pair = h->pair;
     {   // the next ticket is drawn ~2.5 loaded round trips (ticket atomic, table entry, ready counters) before
         // the weight loader runs out of K-blocks
         const double w_bytes = h->n_sub * static_cast<double>(kWTileBytes), a_bytes = h->tile_m * 128.0;
@@ -798,7 +809,7 @@ int lookup_tmap(mlp_pipe* h, TmapCacheEntry* cache, int* next, const void* ptr, 
 // Ticket bookkeeping of one launch over layers [layer_begin, layer_end) (see kernel.cuh, scheduler):
 // CTAs that START on a layer take unit `rank` statically, everyone else draws atomically.
 void set_ticket_params(const mlp_pipe* h, KernelParams& P) {
-    const int b = P.layer_begin, e = P.layer_end, G = h->grid, p = P.producer_ctas;
+    const int b = P.layer_begin, e = P.layer_end, G = h->workers, p = P.producer_ctas;
     for (int l = b; l < e; ++l) {
         const int statics = l == b ? p : (l == b + 1 ? G - p : 0);
         const int arrivals = l == b ? 0 : (l == b + 1 ? p : G);
@@ -814,16 +825,25 @@ int launch(mlp_pipe* h, KernelParams& P, cudaStream_t s) {
     cfg.blockDim = dim3(kThreads);
     cfg.dynamicSmemBytes = h->smem_bytes;
     cfg.stream = s;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     cfg.attrs = nullptr;
     cfg.numAttrs = 0;
-    if (P.pdl_wait) {  // programmatic dependent launch of layer l+1 on layer l (a stronger baseline than the paper's, SURVEY.md NEXT-4)
-        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-        attr[0].val.programmaticStreamSerializationAllowed = 1;
+    if (h->pair) {  // CTA pairs: clusters of 2 (same TPC), required by tcgen05 cta_group::2
+        attr[cfg.numAttrs].id = cudaLaunchAttributeClusterDimension;
+        attr[cfg.numAttrs].val.clusterDim.x = 2;
+        attr[cfg.numAttrs].val.clusterDim.y = 1;
+        attr[cfg.numAttrs].val.clusterDim.z = 1;
         cfg.attrs = attr;
-        cfg.numAttrs = 1;
+        ++cfg.numAttrs;
     }
-    CUDA_TRY(h, cudaLaunchKernelEx(&cfg, mlp_pipe_kernel, P));
+    if (P.pdl_wait) {  // programmatic dependent launch of layer l+1 on layer l (a stronger baseline than the paper's, SURVEY.md NEXT-4)
+        attr[cfg.numAttrs].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[cfg.numAttrs].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        ++cfg.numAttrs;
+    }
+    if (h->pair) CUDA_TRY(h, cudaLaunchKernelEx(&cfg, mlp_pipe_kernel<true>, P));
+    else CUDA_TRY(h, cudaLaunchKernelEx(&cfg, mlp_pipe_kernel<false>, P));
     return MLP_OK;
 }
 
@@ -841,7 +861,7 @@ int install_plan(mlp_pipe* h) {
             CUDA_TRY(h, cudaMalloc(&h->d_table[l], h->table_cap[l] * sizeof(UnitDesc)));
         }
         CUDA_TRY(h, cudaMemcpy(h->d_table[l], h->table[l].data(), n * sizeof(UnitDesc), cudaMemcpyHostToDevice));
-        const size_t ws_bytes = h->split[l] > 1 ? static_cast<size_t>(h->tiles[l]) * h->split[l] * h->n_sub * h->tile_m * kTileN * sizeof(float) : 0;
+        const size_t ws_bytes = h->split[l] > 1 ? static_cast<size_t>(h->tiles[l]) * h->split[l] * (h->pair ? 2 : h->n_sub) * h->tile_m * kTileN * sizeof(float) : 0;
         if (ws_bytes > h->ws_cap[l]) {
             if (h->ws[l]) CUDA_TRY(h, cudaFree(h->ws[l]));
             h->ws[l] = nullptr;
@@ -938,6 +958,11 @@ int create_impl(mlp_pipe** out, int M, int L, const int* widths, int dtype, int 
     h->dev = dev;
     h->num_sms = prop.multiProcessorCount;
     resolve(h);
+    if (h->pair && ((h->tile_m % 32) != 0 || h->grid < 2)) {
+        const int tm = h->tile_m;
+        delete h;
+        return fail(nullptr, MLP_ERR_UNSUPPORTED, "MLP_FLAG_PAIR needs a token tile that is a multiple of 32 (resolved tile_m = %d) and >= 2 SMs", tm);
+    }
 
 #define CREATE_TRY(expr)                                                             \
     do {                                                                             \
@@ -951,7 +976,8 @@ int create_impl(mlp_pipe** out, int M, int L, const int* widths, int dtype, int 
         }                                                                            \
     } while (0)
 
-    CREATE_TRY(cudaFuncSetAttribute(mlp_pipe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(h->smem_bytes)));
+    if (h->pair) CREATE_TRY(cudaFuncSetAttribute(mlp_pipe_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(h->smem_bytes)));
+    else CREATE_TRY(cudaFuncSetAttribute(mlp_pipe_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(h->smem_bytes)));
     for (int l = 0; l < L - 1; ++l) CREATE_TRY(cudaMalloc(&h->H[l], static_cast<size_t>(M) * widths[l + 1] * 2));
     // counters are laid out for 128-row tiles (the larger count), so that the measured search may switch tile_n
     size_t words = 0;
@@ -1012,7 +1038,7 @@ int run_core(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStre
         return fail(h, MLP_ERR_TIMEOUT, "a previous run hit the flag watchdog; the handle has been reset");
     }
     KernelParams P = h->base;
-    if ((rc = lookup_tmap(h, h->cache_x, &h->cache_x_next, X, h->M, h->widths[0], h->tile_m, &P.tm_a[0]))) return rc;
+    if ((rc = lookup_tmap(h, h->cache_x, &h->cache_x_next, X, h->M, h->widths[0], h->pair ? h->tile_m / 2 : h->tile_m, &P.tm_a[0]))) return rc;
     for (int l = 0; l < h->L; ++l)
         if ((rc = lookup_tmap(h, h->cache_w[l], &h->cache_w_next[l], W[l], h->widths[l + 1], h->widths[l], kTileN * h->n_sub, &P.tm_w[l])))
             return rc;
@@ -1039,7 +1065,7 @@ int run_core(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStre
             P.m_end = h->M;
             P.wait_flags = 0;
             P.pdl_wait = (h->mode.flags & MLP_FLAG_PDL) && l > 0 ? 1 : 0;
-            P.producer_ctas = h->grid;
+            P.producer_ctas = h->workers;
             P.epoch_counter = h->epoch + l;
             P.stats = h->stats + static_cast<size_t>(l) * h->grid;
             if ((rc = launch(h, P, s))) return rc;
@@ -1059,7 +1085,7 @@ int run_core(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStre
                 P.m_off = c * rows;
                 P.m_end = (c + 1) * rows;
                 P.wait_flags = 0;
-                P.producer_ctas = h->grid;
+                P.producer_ctas = h->workers;
                 P.epoch_counter = h->epoch + l;
                 P.stats = h->stats + static_cast<size_t>(l) * h->grid;
                 if ((rc = launch(h, P, h->side[l]))) return rc;
@@ -1095,7 +1121,8 @@ int last_span_us(mlp_pipe* h, double* out) {
 int reshape(mlp_pipe* h, int tile_n) {
     h->mode.tile_n = tile_n;
     resolve(h);
-    CUDA_TRY(h, cudaFuncSetAttribute(mlp_pipe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(h->smem_bytes)));
+    if (h->pair) CUDA_TRY(h, cudaFuncSetAttribute(mlp_pipe_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(h->smem_bytes)));
+    else CUDA_TRY(h, cudaFuncSetAttribute(mlp_pipe_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(h->smem_bytes)));
     for (int l = 0; l < kMaxLayers; ++l)
         for (int i = 0; i < kTmapCache; ++i) h->cache_w[l][i].ptr = nullptr;
     return MLP_OK;
@@ -1336,7 +1363,7 @@ int mlp_pipe_stats(mlp_pipe* h, mlp_stats* out, size_t bytes) {
     st.grid = h->grid;
     st.stages = h->stages;
     st.tile_m = h->tile_m;
-    st.tile_n = kTileN * h->n_sub;
+    st.tile_n = kTileN * (h->pair ? 2 : h->n_sub);
     st.producer_ctas = h->producer_ctas;
     for (int l = 0; l < h->L; ++l) {
         st.split_k[l] = h->split[l];
@@ -1368,12 +1395,12 @@ int mlp_pipe_stats(mlp_pipe* h, mlp_stats* out, size_t bytes) {
     bool ok = st.status == 0;
     for (int l = 0; l < h->L && ok; ++l) {
         const unsigned long long e = (h->mode.kind == MLP_CTA_PIPELINED ? ep[0] : ep[l]) / h->grid;
-        const int arrivals = h->mode.kind != MLP_CTA_PIPELINED || l == 0 ? 0 : (l == 1 ? h->producer_ctas : h->grid);
+        const int arrivals = h->mode.kind != MLP_CTA_PIPELINED || l == 0 ? 0 : (l == 1 ? h->producer_ctas : h->workers);
         const uint32_t* tk = cw.data() + (h->ticket[l] - h->counters);
         const uint32_t* ar = cw.data() + (h->arrive[l] - h->counters);
         const uint32_t* rd = cw.data() + (h->ready[l] - h->counters);
         ok = ok && tk[0] == static_cast<uint32_t>(e * static_cast<unsigned long long>(st.units[l] + arrivals));
-        for (int t = 0; t < h->tiles[l] && ok; ++t) {
+        for (int t = 0; t < h->tiles[l] * (h->pair ? 2 : 1) && ok; ++t) {  // (pair mode: counters are per 128-row block)
             ok = ok && ar[t] == (h->split[l] > 1 ? static_cast<uint32_t>(e * h->split[l]) : 0u);
             ok = ok && rd[t] == (l < h->L - 1 ? static_cast<uint32_t>(e * h->ready_inc[l]) : 0u);
         }
@@ -1458,7 +1485,7 @@ int mlp_pipe_plan(int M, int n_layers, const int* widths, const mlp_mode* mode, 
     resolve(&h);
     memset(out, 0, sizeof *out);
     out->tile_m = h.tile_m;
-    out->tile_n = kTileN * h.n_sub;
+    out->tile_n = kTileN * (h.pair ? 2 : h.n_sub);
     out->m_blks = h.m_blks;
     out->stages = h.stages;
     out->a_stages = h.a_stages;

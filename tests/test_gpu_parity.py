@@ -450,3 +450,48 @@ def test_soak_full_size_runs_are_bit_identical(ci, flags, runs):
     st = p.stats()
     assert st.ready_ok == 1 and st.status == 0
     p.close()
+
+
+PAIR = B.MLP_FLAG_PAIR
+
+
+@pytest.mark.parametrize("kw", [dict(kind=P), dict(kind=S), dict(kind=P, split_k=4), dict(kind=P, split_k_layer=[2, 8]), dict(kind=MB, chunks=2),
+                                dict(kind=P, flags=B.MLP_FLAG_DEBUG_DELAY, split_k=2), dict(kind=P, stages=2, a_stages=2), dict(kind=P, grid=2),
+                                dict(kind=P, flags=B.MLP_FLAG_AUTOTUNE)],
+                         ids=[str(i) for i in range(9)])
+def test_cta_pair_mode_exact(kw):
+    """MLP_FLAG_PAIR (tcgen05 cta_group::2, clusters of two; SURVEY.md NEXT-3, PAPER.md:131-133): a pair executes a unit of
+    256 weight rows, each CTA staging its 128 rows and half of the tokens; counters / partials / outputs stay per 128-row
+    block.  Exact-mode bits on cfg 0 and on ragged shapes (odd number of 128-row blocks, several M-blocks, 3 layers)."""
+    kw = dict(kw)
+    kw["flags"] = kw.get("flags", 0) | PAIR
+    check(inputs.get_config(0, "exact"), B.make_mode(**kw))
+    if kw["kind"] != MB:
+        check(inputs.Config("pair_ragged", 96, (200, 392, 136), B.MLP_ACT_RELU, "exact", 4), B.make_mode(**kw))
+        check(inputs.Config("pair_3l_m300", 300, (136, 264, 520, 136), B.MLP_ACT_RELU, "exact", 6), B.make_mode(**kw))
+
+
+def test_cta_pair_mode_full_size_and_protocol():
+    """Pair mode on full sizes (cfg 2: M = 256, sampled rows; cfg 4: the 4-layer chain) and under poison + delays."""
+    sampled_rows_check(2, B.make_mode(P, flags=PAIR), rows=[0, 1, 127, 128, 255])
+    err, st = sampled_rows_check(4, B.make_mode(P, flags=PAIR), rows=[0, 63, 64, 127])
+    assert st.n_layers == 4
+    cfg = inputs.Config("pair_adv", 64, (1024, 4096, 1024), B.MLP_ACT_RELU, "exact", 5)
+    X, Ws, outs, _ = oracle_outs(cfg)
+    Xd, Wd = X.cuda(), [w.cuda() for w in Ws]
+    p = B.MlpPipe(cfg.M, cfg.widths, cfg.act, B.make_mode(P, split_k=4, flags=PAIR | B.MLP_FLAG_DEBUG_DELAY))
+    for _ in range(50):
+        p.poison_hidden(0x7FC0)
+        Y = p.run(Xd, Wd)
+        assert np.array_equal(inputs.as_u16(Y.cpu()), outs[-1])
+    st = p.stats()
+    assert st.ready_ok == 1 and st.status == 0 and st.runs == 50
+    p.close()
+
+
+def test_cta_pair_mode_rejects_unsupported_shapes():
+    with pytest.raises(B.MlpError) as e:
+        B.MlpPipe(16, (64, 128, 128), 0, B.make_mode(P, flags=PAIR))        # tile_m = 16: not a multiple of 32
+    assert e.value.status == B.MLP_ERR_UNSUPPORTED
+    with pytest.raises(B.MlpError):
+        B.MlpPipe(64, (64, 128, 128), 0, B.make_mode(P, flags=PAIR | B.MLP_FLAG_WORKQUEUE))

@@ -15,16 +15,19 @@ SHAPES = [(c.M, tuple(c.widths)) for c in inputs.CONFIGS] + [
 MODES = [
     dict(kind=P), dict(kind=S), dict(kind=MB, chunks=1), dict(kind=P, sm_split=0.5), dict(kind=P, split_k=4),
     dict(kind=P, split_k=3, flags=B.MLP_FLAG_DEBUG_REVERSE), dict(kind=P, tile_n=256, tile_m=64), dict(kind=P, tile_n=128),
-    dict(kind=P, split_k_layer=[2, 9]), dict(kind=S, split_k=16),
+    dict(kind=P, split_k_layer=[2, 9]), dict(kind=S, split_k=16), dict(kind=P, flags=B.MLP_FLAG_PAIR), dict(kind=S, flags=B.MLP_FLAG_PAIR, split_k=3),
 ]
 
 
-def _check_tables(M, widths, plan, tables):
+def _check_tables(M, widths, plan, tables, pair=False):
     L = len(widths) - 1
     rows = M
     assert plan.tile_m % 16 == 0 and 16 <= plan.tile_m <= 256 and plan.tile_n in (128, 256)
     assert plan.m_blks * plan.tile_m >= rows
-    assert plan.acc_stages * (plan.tile_n // 128) * plan.tile_m <= 512, "accumulator ring must fit the 512 TMEM columns"
+    acc_cols = plan.tile_m if pair else (plan.tile_n // 128) * plan.tile_m   # pair mode: each CTA keeps its own 128 rows
+    assert plan.acc_stages * acc_cols <= 512, "accumulator ring must fit the 512 TMEM columns"
+    if pair:
+        assert plan.tile_n == 256 and plan.tile_m % 32 == 0 and plan.grid % 2 == 0
     assert plan.smem_bytes <= 227 * 1024
     for l in range(L):
         K, N = widths[l], widths[l + 1]
@@ -80,8 +83,13 @@ def test_unit_tables_are_a_valid_schedule(M, widths, mode):
     m = B.make_mode(**kw)
     if kw.get("tile_m") and kw["tile_m"] * 2 > 512:
         pytest.skip("shape not supported")
+    pair = bool(kw.get("flags", 0) & B.MLP_FLAG_PAIR)
+    if pair and (-(-min(M, 256) // 16) * 16) % 32 != 0 and M <= 256:
+        pytest.skip("pair mode needs a token tile that is a multiple of 32")
     plan, tables = B.plan(M, widths, m, num_sms=148)
-    _check_tables(M, widths, plan, tables)
+    if pair and plan.tile_m % 32 != 0:
+        pytest.skip("pair mode needs a token tile that is a multiple of 32")
+    _check_tables(M, widths, plan, tables, pair=pair)
     assert plan.model_us > 0
 
 
