@@ -495,3 +495,24 @@ def test_cta_pair_mode_rejects_unsupported_shapes():
     assert e.value.status == B.MLP_ERR_UNSUPPORTED
     with pytest.raises(B.MlpError):
         B.MlpPipe(64, (64, 128, 128), 0, B.make_mode(P, flags=PAIR | B.MLP_FLAG_WORKQUEUE))
+
+
+@pytest.mark.parametrize("kw", [dict(kind=S, flags=PAIR | B.MLP_FLAG_PDL, split_k=2), dict(kind=P, flags=PAIR, sm_split=0.5, split_k=4),
+                                dict(kind=P, flags=PAIR, sm_split=0.25, split_k=2),
+                                dict(kind=P, flags=PAIR | B.MLP_FLAG_DEBUG_REVERSE | B.MLP_FLAG_DEBUG_DELAY, split_k=4),
+                                dict(kind=P, flags=PAIR | B.MLP_FLAG_ACQUIRE_LOADS, split_k=4), dict(kind=P, flags=PAIR, grid=146),
+                                dict(kind=MB, chunks=2, flags=PAIR)], ids=[str(i) for i in range(7)])
+def test_cta_pair_mode_with_other_options(kw):
+    """Pair mode combined with the other launch options (PDL, consumer-first pairs, reversed / delayed producers, literal
+    acquire polls, a smaller even grid, micro-batches), H poisoned before every run."""
+    cfg = inputs.Config("pair_opts", 64, (1024, 4096, 1024), B.MLP_ACT_RELU, "exact", 5)
+    X, Ws, outs, _ = oracle_outs(cfg)
+    Xd, Wd = X.cuda(), [w.cuda() for w in Ws]
+    p = B.MlpPipe(cfg.M, cfg.widths, cfg.act, B.make_mode(**kw))
+    for _ in range(5):
+        p.poison_hidden(0x7FC0)
+        Y = p.run(Xd, Wd)
+        assert np.array_equal(inputs.as_u16(Y.cpu()), outs[-1])
+    st = p.stats()
+    assert st.ready_ok == 1 and st.status == 0
+    p.close()
