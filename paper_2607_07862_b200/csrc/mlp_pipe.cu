@@ -266,12 +266,29 @@ struct Planner {
         bool ksm;
         if (mode == kReduceUnits) ksm = !force_tile_major && !producer_in_launch(l) && consumer_in_launch(l);
         else ksm = !force_tile_major && !producer_in_launch(l) && sp > 4;
+        // Tile order inside a layer.  Few M-blocks: M-block-major (tile index order).  Many M-blocks (M in the thousands, the
+        // paper's tensor-bound regime): groups of kRasterM M-blocks, weight-tile-major inside a group, so that the workers
+        // running side by side share a handful of weight tiles through L2 instead of streaming one each from HBM (at
+        // M = 4096, 8192^2 the M-block-major order pulls every weight tile once per M-block: 4.5 TB/s of HBM traffic), while
+        // groups of M-blocks still complete one after the other for the consumer layer.
+        constexpr int kRasterM = 8;
+        std::vector<int> order(tiles);
+        {
+            const int nb = tiles / h->m_blks;
+            int i = 0;
+            if (h->m_blks >= 4 && !getenv("MLP_PIPE_NO_RASTER"))
+                for (int mg = 0; mg < h->m_blks; mg += kRasterM)
+                    for (int n = 0; n < nb; ++n)
+                        for (int mb = mg; mb < std::min(h->m_blks, mg + kRasterM); ++mb) order[i++] = mb * nb + n;
+            else
+                for (int t = 0; t < tiles; ++t) order[i++] = t;
+        }
         if (ksm) {
             for (int ks = 0; ks < sp; ++ks)
-                for (int t = 0; t < tiles; ++t) mma(t, ks);
+                for (int t = 0; t < tiles; ++t) mma(order[t], ks);
         } else {
             for (int t = 0; t < tiles; ++t)
-                for (int ks = 0; ks < sp; ++ks) mma(t, ks);
+                for (int ks = 0; ks < sp; ++ks) mma(order[t], ks);
         }
         if (reverse) std::reverse(out.begin(), out.end());
         if (mode != kReduceUnits) return;
@@ -300,13 +317,13 @@ struct Planner {
         int next_red = 0;
         for (int i = 0; i < static_cast<int>(out.size()); ++i) {
             merged.push_back(out[i]);
-            while (next_red < tiles && (next_red + 1) * sp - 1 + delay <= i) {
-                for (int c = 0; c < chunks; ++c) merged.push_back(red(next_red, c));
+            while (next_red < tiles && (next_red + 1) * sp - 1 + delay <= i) {  // (next_red counts tiles in ticket order)
+                for (int c = 0; c < chunks; ++c) merged.push_back(red(order[next_red], c));
                 ++next_red;
             }
         }
         for (; next_red < tiles; ++next_red)
-            for (int c = 0; c < chunks; ++c) merged.push_back(red(next_red, c));
+            for (int c = 0; c < chunks; ++c) merged.push_back(red(order[next_red], c));
         out.swap(merged);
     }
 
@@ -981,13 +998,14 @@ int create_impl(mlp_pipe** out, int M, int L, const int* widths, int dtype, int 
     for (int l = 0; l < L - 1; ++l) CREATE_TRY(cudaMalloc(&h->H[l], static_cast<size_t>(M) * widths[l + 1] * 2));
     // counters are laid out for 128-row tiles (the larger count), so that the measured search may switch tile_n
     size_t words = 0;
-    for (int l = 0; l < L; ++l) words += 32 + 2 * static_cast<size_t>(round_up(ceil_div(widths[l + 1], kTileN) * h->m_blks, 32));
+    // (2 * ceil(N / 256) blocks per M-block: pair mode indexes a phantom block when N / 128 is odd)
+    for (int l = 0; l < L; ++l) words += 32 + 2 * static_cast<size_t>(round_up(2 * ceil_div(widths[l + 1], 2 * kTileN) * h->m_blks, 32));
     h->counters_words = words;
     CREATE_TRY(cudaMalloc(&h->counters, words * sizeof(uint32_t)));
     {
         uint32_t* p = h->counters;
         for (int l = 0; l < L; ++l) {
-            const int t128 = round_up(ceil_div(widths[l + 1], kTileN) * h->m_blks, 32);
+            const int t128 = round_up(2 * ceil_div(widths[l + 1], 2 * kTileN) * h->m_blks, 32);
             h->ticket[l] = p;  // own 128-byte line
             p += 32;
             h->arrive[l] = p;

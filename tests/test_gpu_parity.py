@@ -516,3 +516,30 @@ def test_cta_pair_mode_with_other_options(kw):
     st = p.stats()
     assert st.ready_ok == 1 and st.status == 0
     p.close()
+
+
+@pytest.mark.parametrize("kw", [dict(kind=P), dict(kind=S), dict(kind=P, split_k=2), dict(kind=P, split_k_layer=[3, 2], tile_m=128),
+                                dict(kind=P, flags=PAIR), dict(kind=P, flags=PAIR, split_k=2, tile_m=64), dict(kind=MB, chunks=2)],
+                         ids=[str(i) for i in range(7)])
+def test_many_m_blocks_rasterised_order(kw):
+    """M in the thousands (the paper's regime): >= 4 M-blocks, so tiles are handed out in groups of M-blocks,
+    weight-tile-major inside a group (L2 reuse of the weight tiles) -- with K-splits the reduce units must still follow the
+    slices of their tile.  Exact mode, every element, incl. a ragged last M-block."""
+    cfg = inputs.Config("many_m", 1096, (256, 640, 384), B.MLP_ACT_RELU, "exact", 31)
+    st = check(cfg, B.make_mode(**kw))
+    if kw["kind"] != MB:
+        assert st.units[0] >= 4 * 3
+
+
+def test_paper_shape_sampled_rows():
+    """The paper's own workload shape at its smallest M (2 layers, no activation, 8192 x 8192 weights,
+    M = 1024): sampled token rows against the oracle, CTA_PIPELINED with and without CTA pairs."""
+    cfg = inputs.Config("paper_1024", 1024, (8192, 8192, 8192), B.MLP_ACT_NONE, "normal", 7)
+    X, Ws = inputs.make_inputs(cfg)
+    rows = [0, 255, 256, 777, 1023]
+    outs, _ = oracle.mlp_chain(inputs.as_u16(X)[rows].copy(), [inputs.as_u16(w) for w in Ws], cfg.act)
+    for mode in (B.make_mode(P), B.make_mode(P, flags=PAIR)):
+        got, hs, st = run_gpu(cfg, mode, X, Ws)
+        assert st.status == 0 and st.ready_ok == 1
+        e = oracle.rel_err(got[rows], outs[-1])
+        assert e["nan"] == 0 and e["err"] <= TOL, e
