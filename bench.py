@@ -43,6 +43,11 @@ def parse_args():
     ap.add_argument("--split-k", type=str, default="", help="comma list, per layer")
     ap.add_argument("--no-extras", action="store_true", help="skip the side measurements (other modes, e2e, cpu baseline)")
     ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--shape", type=str, default="",
+                    help="M,K,N1,...: a custom chain instead of a BASELINE.json config (e.g. the paper's own workload 16384,8192,8192,8192)")
+    ap.add_argument("--act", type=int, default=-1, help="activation for --shape: 0 none, 1 ReLU, 2 GeLU-tanh")
+    ap.add_argument("--pair", action="store_true", help="CTA pairs / 2-CTA MMA (MLP_FLAG_PAIR)")
+    ap.add_argument("--cublas-ref", action="store_true", help="also time the torch.matmul chain (cuBLAS) on the same inputs: context only")
     ap.add_argument("--no-autotune", action="store_true",
                     help="use the modelled plan instead of the measured plan search of the first (warm-up) run")
     return ap.parse_args()
@@ -147,7 +152,8 @@ def make_mode(B, args, n_layers):
     kind = {"pipelined": B.MLP_CTA_PIPELINED, "sequential": B.MLP_SEQUENTIAL, "microbatch": B.MLP_MICROBATCH}[args.mode]
     split = [int(x) for x in args.split_k.split(",")] if args.split_k else []
     return B.make_mode(kind, chunks=args.chunks if kind == B.MLP_MICROBATCH else 0, sm_split=args.sm_split,
-                       stages=args.stages, split_k_layer=split, flags=0 if args.no_autotune else B.MLP_FLAG_AUTOTUNE)
+                       stages=args.stages, split_k_layer=split,
+                       flags=(0 if args.no_autotune else B.MLP_FLAG_AUTOTUNE) | (B.MLP_FLAG_PAIR if args.pair else 0))
 
 
 def device_inputs(torch, cfg, n_sets):
@@ -275,6 +281,10 @@ def main():
         dist = dist_mod
 
     cfg = inputs.CONFIGS[args.config]
+    if args.shape:
+        dims = [int(x) for x in args.shape.split(",")]
+        cfg = inputs.Config("custom_" + "x".join(map(str, dims)), dims[0], tuple(dims[1:]), args.act if args.act >= 0 else 0, "normal", 7,
+                            "custom shape (--shape)")
     mode = make_mode(B, args, cfg.n_layers)
     X, sets = device_inputs(torch, cfg, N_WEIGHT_SETS)
     Y = torch.empty((cfg.M, cfg.widths[-1]), dtype=torch.bfloat16, device="cuda")
@@ -302,12 +312,21 @@ def main():
                 "algorithmic_bytes_per_launch": bytes_per_launch, "avg_launch_us": kern_us,
                 "roofline_us_at_peak": alg_bytes / peak / 1e3, "tflops": cfg.flops / value / 1e6}
 
+    # a tensor-bound shape (the paper's own workload via --shape): roofline against the measured cuBLAS bf16 rate instead
+    tpeak = float(mp.get("bf16_tflops_sustained", mp.get("bf16_tflops", 1590.0))) if mp else 1590.0
+    if cfg.flops / (tpeak * 1e6) > alg_bytes / peak / 1e3:
+        achieved_tf = cfg.flops / lat["mean"] / 1e6
+        roofline = {"bound": "tensor", "achieved": achieved_tf, "peak": tpeak, "unit": "TFLOP/s", "frac": achieved_tf / tpeak, "traffic": None,
+                    "peak_source": "measured (MEASURED_PEAKS.json bf16_tflops_sustained)" if mp else "fallback (B200_PROFILING.md 1.59 PFLOP/s)",
+                    "kernel": "mlp_pipe_kernel", "flops_per_step": cfg.flops, "avg_step_us": lat["mean"],
+                    "roofline_us_at_peak": cfg.flops / (tpeak * 1e6), "tflops": cfg.flops / value / 1e6}
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16 in/out, fp32 accumulate", "data": "synthetic",
-        "config": {"workload": f"BASELINE.json configs[{args.config}]: {cfg.name} M={cfg.M} widths={list(cfg.widths)} act={cfg.act}",
-                   "mode": args.mode, "grid": st.grid, "tile_m": st.tile_m, "stages": st.stages,
+        "config": {"workload": (f"custom: M={cfg.M} widths={list(cfg.widths)} act={cfg.act}" if args.shape else
+                                f"BASELINE.json configs[{args.config}]: {cfg.name} M={cfg.M} widths={list(cfg.widths)} act={cfg.act}"),
+                   "mode": args.mode, "cta_pairs": bool(args.pair), "grid": st.grid, "tile_m": st.tile_m, "stages": st.stages,
                    "split_k": list(st.split_k)[:cfg.n_layers], "sm_split": args.sm_split, "tile_n": st.tile_n,
                    "plan": "modelled" if args.no_autotune else "autotuned on the first warm-up run (MLP_FLAG_AUTOTUNE)",
                    "l2": f"inputs larger than L2: {N_WEIGHT_SETS} rotating weight sets of {alg_bytes / 1e6:.0f} MB, no weight reuse across steps",
@@ -315,6 +334,28 @@ def main():
         "latency_us": lat, "clocks": clocks, "gpu_launches": args.steps * launches_per_step, "roofline": roofline,
         "flag_stall_cycles_max": int(st.flag_stall_cycles_max),
     }
+    if args.cublas_ref and rank == 0:
+        def chain():
+            a = X
+            for l, w in enumerate(sets[0]):
+                a = torch.matmul(a, w.t())
+                if l < cfg.n_layers - 1 and cfg.act == 2:
+                    a = torch.nn.functional.gelu(a, approximate="tanh")
+                elif l < cfg.n_layers - 1 and cfg.act == 1:
+                    a = torch.relu(a)
+            return a
+        for _ in range(3):
+            chain()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ts = []
+        for _ in range(10):
+            e0.record()
+            chain()
+            e1.record()
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1) * 1e3)
+        ts.sort()
+        line["cublas_chain_us"] = {"median": ts[len(ts) // 2], "note": "torch.matmul chain on one weight set: library context, not part of the metric"}
     if rank == 0 and not args.no_extras:
         line.update(extras(torch, B, inputs, cfg, args, X, sets, Y, with_cpu=(world == 1)))
     if dist is not None:
