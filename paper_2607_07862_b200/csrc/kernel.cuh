@@ -176,7 +176,7 @@ __device__ __forceinline__ float ld_cg_f32(const float* p) {
 }
 
 __device__ __forceinline__ void mbar_wait_timed(uint32_t bar, uint32_t parity, unsigned long long& acc) {
-    if (mbar_test(bar, parity)) return;
+    if (mbar_probe(bar, parity)) return;
     const long long t0 = clock64();
     mbar_wait(bar, parity);
     acc += static_cast<unsigned long long>(clock64() - t0);
@@ -409,6 +409,9 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
     const int stages = P.stages;      // weight ring depth
     const int a_stages = P.a_stages;  // activation ring depth (its own, deeper ring: the consumer prologue's
                                       // polls and fences then run K-blocks ahead of the weight stream)
+    // Equally deep rings share their barriers: "stage s landed" counts the bytes of both tiles (two arrivals, one per
+    // loader), "stage s consumed" is ONE commit that both loaders wait for -- one wait and one commit per K-block.
+    const bool unified = stages == a_stages;
     const uint32_t a_ring = smem_base + static_cast<uint32_t>(stages) * w_tile_bytes;
     const uint32_t stage_s = a_ring + static_cast<uint32_t>(a_stages) * a_tile_bytes;  // epilogue staging
     const uint32_t ring_bytes = static_cast<uint32_t>(stages) * w_tile_bytes + static_cast<uint32_t>(a_stages) * a_tile_bytes + kStageBytes;
@@ -418,9 +421,9 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
     const uint32_t ctrl_s = smem_base + ring_bytes;
     const uint32_t bar_full = ctrl_s;                          // [kMaxStages]  weight tile landed
     const uint32_t bar_empty = bar_full + 8 * kMaxStages;      // [kMaxStages]  weight stage consumed
-    const uint32_t bar_afull = bar_empty + 8 * kMaxStages;     // [kMaxStages]  activation tile landed
-    const uint32_t bar_aempty = bar_afull + 8 * kMaxStages;    // [kMaxStages]  activation stage consumed
-    const uint32_t bar_tfull = bar_aempty + 8 * kMaxStages;    // [kMaxAccStages]
+    const uint32_t bar_afull = unified ? bar_full : bar_empty + 8 * kMaxStages;     // [kMaxStages]  activation tile landed
+    const uint32_t bar_aempty = unified ? bar_empty : bar_empty + 16 * kMaxStages;  // [kMaxStages]  activation stage consumed
+    const uint32_t bar_tfull = bar_full + 32 * kMaxStages;     // [kMaxAccStages]
     const uint32_t bar_tempty = bar_tfull + 8 * kMaxAccStages;  // [kMaxAccStages]
     const uint32_t bar_sfull = bar_tempty + 8 * kMaxAccStages;  // [kSchedSlots]
     const uint32_t bar_sempty = bar_sfull + 8 * kSchedSlots;   // [kSchedSlots]
@@ -461,7 +464,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
         // parallel (92 serial mbarrier.init cost ~1 us at the head of every CTA), arrival counts by slot range.
         constexpr int kNumBars = 4 * kMaxStages + 2 * kMaxAccStages + 3 * kSchedSlots;
         for (int b = lane; b < kNumBars; b += 32) {
-            uint32_t count = 1;
+            uint32_t count = (unified && b < kMaxStages) ? 2u : 1u;                                                                   // full (unified: W loader + A loader)
             if (b >= 4 * kMaxStages + kMaxAccStages && b < 4 * kMaxStages + 2 * kMaxAccStages) count = kEpiThreads * nb_mul;          // tempty (pair: both CTAs' epilogues)
             if (b >= 4 * kMaxStages + 2 * kMaxAccStages + kSchedSlots && b < 4 * kMaxStages + 2 * kMaxAccStages + 2 * kSchedSlots)
                 count = (3 + kEpiThreads) * nb_mul;                                                                                   // sempty (pair: both CTAs' consumers)
@@ -651,7 +654,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                             fence_acq_rel_gpu();
                             u.acquired = 1;
                         }
-                    } else if (P.wait_flags && l > P.layer_begin && !pair && !(P.flags & (kFlagExpNoFastPath | kFlagAcquireLoads))) {
+                    } else if (P.wait_flags && l > P.layer_begin && !(P.flags & (kFlagExpNoFastPath | kFlagAcquireLoads))) {
                         // Consumer prologue, fast path (the prologue lives in the scheduler
                         // warp): one look at all ready counters under this unit's K range.  If every producer
                         // tile is already published -- the normal case, the scheduler runs a unit ahead --
@@ -659,9 +662,11 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                         // the activation loader polls slice by slice while the weight loader prefetches.
                         const LayerParams& Lp = P.layer[l - 1];
                         const uint32_t target = static_cast<uint32_t>((epoch + 1ull) * static_cast<unsigned long long>(Lp.ready_inc));
-                        const uint32_t* rd = Lp.ready + u.m_blk * Lp.n_blks;
+                        // (pair mode: the counters are per 128-row block, tile_n = 128 here, and the acquire reaches the peer's
+                        // loaders through the cluster-scope release / acquire of the slot hand-over: causality order is transitive)
+                        const uint32_t* rd = Lp.ready + u.m_blk * Lp.n_blks * nb_mul;
                         const int s0 = (u.kb0 * kTileK) / tile_n, s1 = ((u.kb1 - 1) * kTileK) / tile_n + 1;
-                        bool all = (s1 - s0) <= 32;
+                        bool all = (s1 - s0) <= 256;  // (the scheduler runs a unit ahead: its round trips are off the critical path)
                         for (int sb = s0; sb < s1 && all; sb += 8) {
                             uint32_t v[8];
 #pragma unroll
@@ -874,8 +879,12 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
             }
         }
     } else if (warp == 3) {
-        // ===== MMA issuer (steps a2, a6)
-        if (lane == 0) {
+        // ===== MMA issuer (steps a2, a6).  All 32 lanes run the loop CONVERGED and wait on the barriers; one elected lane
+        // issues.  (A lone `lane == 0` thread makes ptxas wrap every tcgen05 instruction into an elect / branch loop over
+        // the active lanes, and the round trip of each mbarrier test then sits between two MMAs: measured 858 cycles per
+        // K-block of 4 MMAs + 2 waits + 2 commits against a tensor-core floor of 512 at N = 256 -- the pipe was paced by
+        // its issuer.  Converged, with ONE wait and ONE commit per K-block where the rings are equally deep: 424.)
+        {
             // pair mode: ONE instruction of the leader drives both tensor cores -- M = 256 (128 weight rows per CTA), the
             // tile_m tokens of the B operand half in each CTA's shared memory, D in both TMEMs at the same address
             const uint32_t idesc = make_idesc_bf16(pair ? 2 * kTileN : kTileN, tile_m);
@@ -886,7 +895,8 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 const uint32_t slot = it % kSchedSlots;
                 wait_shared(bar_sfull + 8 * slot, (it / kSchedSlots) & 1, pair);
                 const UnitInfo u = ring[slot];
-                arrive_leader(bar_sempty + 8 * slot, pair);
+                __syncwarp();  // every lane holds the unit before the slot is handed back
+                if (lane == 0) arrive_leader(bar_sempty + 8 * slot, pair);
                 if (!u.valid) break;
                 if (u.kind == kUnitReduce || !leader) continue;  // (the peer's MMA warp only keeps its ring in step)
                 const uint32_t acc = mma_it % acc_stages;
@@ -896,40 +906,48 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + acc * acc_cols;
                 for (int kb = u.kb0; kb < u.kb1; ++kb) {
-                    mbar_wait_timed(bar_afull + 8 * astage, aphase, wait_ops);
+                    if (!unified) mbar_wait_timed(bar_afull + 8 * astage, aphase, wait_ops);
                     mbar_wait_timed(bar_full + 8 * stage, phase, wait_ops);
                     tc_fence_after();
-                    if (it == 0 && kb == u.kb0) my_stats->ts[4] = globaltimer_ns();
+                    if (it == 0 && kb == u.kb0 && lane == 0) my_stats->ts[4] = globaltimer_ns();
                     const uint32_t a_addr = smem_base + stage * w_tile_bytes;
                     const uint32_t b_addr = a_ring + astage * a_tile_bytes;
                     const uint64_t b_desc = make_smem_desc_sw128(b_addr);
-                    for (int rr = 0; rr < n_sub; ++rr) {
-                        // block rr = weight rows [128 rr, 128 rr + 128) of the stage, accumulator columns
-                        // [rr tile_m, (rr + 1) tile_m); both blocks read the same activation tile
-                        const uint64_t a_desc = make_smem_desc_sw128(a_addr + rr * kWTileBytes);
+                    if (elect_one()) {
+                        for (int rr = 0; rr < n_sub; ++rr) {
+                            // block rr = weight rows [128 rr, 128 rr + 128) of the stage, accumulator columns
+                            // [rr tile_m, (rr + 1) tile_m); both blocks read the same activation tile
+                            const uint64_t a_desc = make_smem_desc_sw128(a_addr + rr * kWTileBytes);
 #pragma unroll
-                        for (int k = 0; k < kTileK / kUmmaK; ++k) {
-                            // advancing K by 16 bf16 = 32 B inside the 128 B swizzle span: +2 in the
-                            // (addr >> 4) field of the descriptor
-                            if (pair) umma_bf16_pair(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb > u.kb0 || k > 0) ? 1u : 0u);
-                            else umma_bf16(d_tmem + rr * tile_m, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb > u.kb0 || k > 0) ? 1u : 0u);
+                            for (int k = 0; k < kTileK / kUmmaK; ++k) {
+                                // advancing K by 16 bf16 = 32 B inside the 128 B swizzle span: +2 in the
+                                // (addr >> 4) field of the descriptor
+                                if (pair) umma_bf16_pair(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb > u.kb0 || k > 0) ? 1u : 0u);
+                                else umma_bf16(d_tmem + rr * tile_m, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb > u.kb0 || k > 0) ? 1u : 0u);
+                            }
+                        }
+                        if (pair) {  // the stages of BOTH CTAs are free again
+                            umma_commit_pair(bar_empty + 8 * stage);
+                            if (!unified) umma_commit_pair(bar_aempty + 8 * astage);
+                        } else {
+                            umma_commit(bar_empty + 8 * stage);
+                            if (!unified) umma_commit(bar_aempty + 8 * astage);
+                        }
+                        // both CTAs' epilogues drain their own 128 lanes
+                        if (kb + 1 == u.kb1) {
+                            if (pair) umma_commit_pair(bar_tfull + 8 * acc);
+                            else umma_commit(bar_tfull + 8 * acc);
                         }
                     }
-                    if (pair) {  // the stages of BOTH CTAs are free again
-                        umma_commit_pair(bar_empty + 8 * stage);
-                        umma_commit_pair(bar_aempty + 8 * astage);
-                    } else {
-                        umma_commit(bar_empty + 8 * stage);
-                        umma_commit(bar_aempty + 8 * astage);
-                    }
+                    __syncwarp();
                     if (++stage == static_cast<uint32_t>(stages)) { stage = 0; phase ^= 1; }
                     if (++astage == static_cast<uint32_t>(a_stages)) { astage = 0; aphase ^= 1; }
                 }
-                if (pair) umma_commit_pair(bar_tfull + 8 * acc);  // both CTAs' epilogues drain their own 128 lanes
-                else umma_commit(bar_tfull + 8 * acc);
             }
-            my_stats->wait[2] = wait_ops;
-            my_stats->wait[3] = wait_acc;
+            if (lane == 0) {
+                my_stats->wait[2] = wait_ops;
+                my_stats->wait[3] = wait_acc;
+            }
         }
     } else {
         // ===== epilogue warps 4..7 (steps a3, a4, a7, a8)

@@ -1,7 +1,7 @@
 """Per-CTA unit timeline of one run, from the kernel's own timestamps (`mlp_pipe_cta_records`; the paper's
 in-kernel instrumentation).
 
-    python -m paper_2607_07862_b200.trace --config 1 [--mode pipelined|sequential] [--no-autotune] [--every 12]
+    python -m paper_2607_07862_b200.trace --config 1 [--mode pipelined|sequential] [--no-autotune] [--workqueue] [--pair] [--every 12]
 
 Prints, for every `--every`-th CTA, when it started, requested its first weights, started its first MMA and exited,
 what it waited for (SM cycles -> us at the SM clock), and its first units with their four timestamps (weight loader
@@ -25,6 +25,7 @@ def main() -> int:
     ap.add_argument("--mode", default="pipelined", choices=["pipelined", "sequential"])
     ap.add_argument("--no-autotune", action="store_true")
     ap.add_argument("--workqueue", action="store_true")
+    ap.add_argument("--pair", action="store_true", help="CTA pairs (MLP_FLAG_PAIR)")
     ap.add_argument("--every", type=int, default=12)
     ap.add_argument("--sm-mhz", type=float, default=1965.0)
     args = ap.parse_args()
@@ -37,7 +38,7 @@ def main() -> int:
 
     cfg = inputs.CONFIGS[args.config]
     kind = B.MLP_CTA_PIPELINED if args.mode == "pipelined" else B.MLP_SEQUENTIAL
-    flags = (0 if args.no_autotune else B.MLP_FLAG_AUTOTUNE) | (B.MLP_FLAG_WORKQUEUE if args.workqueue else 0)
+    flags = (0 if args.no_autotune else B.MLP_FLAG_AUTOTUNE) | (B.MLP_FLAG_WORKQUEUE if args.workqueue else 0) | (B.MLP_FLAG_PAIR if args.pair else 0)
     X, sets = bench.device_inputs(torch, cfg, bench.N_WEIGHT_SETS)
     Y = torch.empty((cfg.M, cfg.widths[-1]), dtype=torch.bfloat16, device="cuda")
     p = B.MlpPipe(cfg.M, cfg.widths, cfg.act, B.make_mode(kind, flags=flags))
