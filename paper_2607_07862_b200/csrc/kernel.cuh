@@ -888,6 +888,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
             // pair mode: ONE instruction of the leader drives both tensor cores -- M = 256 (128 weight rows per CTA), the
             // tile_m tokens of the B operand half in each CTA's shared memory, D in both TMEMs at the same address
             const uint32_t idesc = make_idesc_bf16(pair ? 2 * kTileN : kTileN, tile_m);
+            const uint32_t desc_hi = static_cast<uint32_t>(make_smem_desc_sw128(0) >> 32);
             uint32_t stage = 0, phase = 0, astage = 0, aphase = 0;
             unsigned long long wait_ops = 0, wait_acc = 0;
             uint32_t mma_it = 0;  // MMA units so far: picks the accumulator (the epilogue warps count alike)
@@ -910,22 +911,15 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                     mbar_wait_timed(bar_full + 8 * stage, phase, wait_ops);
                     tc_fence_after();
                     if (it == 0 && kb == u.kb0 && lane == 0) my_stats->ts[4] = globaltimer_ns();
-                    const uint32_t a_addr = smem_base + stage * w_tile_bytes;
-                    const uint32_t b_addr = a_ring + astage * a_tile_bytes;
-                    const uint64_t b_desc = make_smem_desc_sw128(b_addr);
+                    // operand descriptors: low word = (address >> 4) | LBO field, high word common (ptx.cuh)
+                    const uint32_t a_lo = (((smem_base + stage * w_tile_bytes) & 0x3ffffu) >> 4) | (1u << 16);
+                    const uint32_t b_lo = (((a_ring + astage * a_tile_bytes) & 0x3ffffu) >> 4) | (1u << 16);
                     if (elect_one()) {
-                        for (int rr = 0; rr < n_sub; ++rr) {
-                            // block rr = weight rows [128 rr, 128 rr + 128) of the stage, accumulator columns
-                            // [rr tile_m, (rr + 1) tile_m); both blocks read the same activation tile
-                            const uint64_t a_desc = make_smem_desc_sw128(a_addr + rr * kWTileBytes);
-#pragma unroll
-                            for (int k = 0; k < kTileK / kUmmaK; ++k) {
-                                // advancing K by 16 bf16 = 32 B inside the 128 B swizzle span: +2 in the
-                                // (addr >> 4) field of the descriptor
-                                if (pair) umma_bf16_pair(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb > u.kb0 || k > 0) ? 1u : 0u);
-                                else umma_bf16(d_tmem + rr * tile_m, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb > u.kb0 || k > 0) ? 1u : 0u);
-                            }
-                        }
+                        // block rr = weight rows [128 rr, 128 rr + 128) of the stage, accumulator columns
+                        // [rr tile_m, (rr + 1) tile_m); both blocks read the same activation tile
+                        const uint32_t accum = kb > u.kb0 ? 1u : 0u;
+                        umma_bf16_kblock<pair>(d_tmem, a_lo, b_lo, desc_hi, idesc, accum);
+                        if (!pair && n_sub == 2) umma_bf16_kblock<false>(d_tmem + tile_m, a_lo + (kWTileBytes >> 4), b_lo, desc_hi, idesc, accum);
                         if (pair) {  // the stages of BOTH CTAs are free again
                             umma_commit_pair(bar_empty + 8 * stage);
                             if (!unified) umma_commit_pair(bar_aempty + 8 * astage);

@@ -174,6 +174,47 @@ __device__ __forceinline__ void umma_bf16(uint32_t d_tmem, uint64_t a_desc, uint
         ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
         : "memory");
 }
+// One 64-element K-block = four K = 16 MMAs on descriptors that advance by 32 B (+2 in the addr >> 4 field) inside the 128 B
+// swizzle span, in ONE asm block: ptxas otherwise rebuilds every 64-bit descriptor with uniform-datapath ALU code between
+// the MMAs.  a_lo / b_lo = low words of the operand descriptors, hi = their common high word; `first` = 0 makes the first
+// MMA overwrite the accumulator.
+template <bool kPairMma>
+__device__ __forceinline__ void umma_bf16_kblock(uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo, uint32_t hi, uint32_t idesc,
+                                                 uint32_t accumulate) {
+    if constexpr (kPairMma) {
+        asm volatile(
+            "{\n\t.reg .pred p, q;\n\t.reg .b64 da, db;\n\t"
+            "setp.ne.b32 p, %5, 0;\n\t"
+            "setp.eq.b32 q, 0, 0;\n\t"
+            "mov.b64 da, {%1, %3};\n\t"
+            "mov.b64 db, {%2, %3};\n\t"
+            "tcgen05.mma.cta_group::2.kind::f16 [%0], da, db, %4, p;\n\t"
+            "add.s64 da, da, 2;\n\tadd.s64 db, db, 2;\n\t"
+            "tcgen05.mma.cta_group::2.kind::f16 [%0], da, db, %4, q;\n\t"
+            "add.s64 da, da, 2;\n\tadd.s64 db, db, 2;\n\t"
+            "tcgen05.mma.cta_group::2.kind::f16 [%0], da, db, %4, q;\n\t"
+            "add.s64 da, da, 2;\n\tadd.s64 db, db, 2;\n\t"
+            "tcgen05.mma.cta_group::2.kind::f16 [%0], da, db, %4, q;\n\t}"
+            ::"r"(d_tmem), "r"(a_lo), "r"(b_lo), "r"(hi), "r"(idesc), "r"(accumulate)
+            : "memory");
+    } else {
+        asm volatile(
+            "{\n\t.reg .pred p, q;\n\t.reg .b64 da, db;\n\t"
+            "setp.ne.b32 p, %5, 0;\n\t"
+            "setp.eq.b32 q, 0, 0;\n\t"
+            "mov.b64 da, {%1, %3};\n\t"
+            "mov.b64 db, {%2, %3};\n\t"
+            "tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %4, p;\n\t"
+            "add.s64 da, da, 2;\n\tadd.s64 db, db, 2;\n\t"
+            "tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %4, q;\n\t"
+            "add.s64 da, da, 2;\n\tadd.s64 db, db, 2;\n\t"
+            "tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %4, q;\n\t"
+            "add.s64 da, da, 2;\n\tadd.s64 db, db, 2;\n\t"
+            "tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %4, q;\n\t}"
+            ::"r"(d_tmem), "r"(a_lo), "r"(b_lo), "r"(hi), "r"(idesc), "r"(accumulate)
+            : "memory");
+    }
+}
 // mbarrier arrives once every MMA issued so far by this thread has completed
 // (implies tcgen05.fence::before_thread_sync).
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
