@@ -706,7 +706,8 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
             }
         }
     } else if (warp == 1) {
-        // ===== W loader
+        // ===== W loader (one thread: measured, the converged form of the other roles is SLOWER here -- paper workload with
+        // pairs 1487 vs 1445 us, cfg 1 55.6 vs 53.4 us)
         if (lane == 0) {
             const uint64_t pol = policy_evict_first();
             const bool hint = !(P.flags & kFlagNoEvictFirst);
@@ -776,7 +777,8 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
         }
     } else if (warp == 2) {
         // ===== A loader = consumer prologue (step a5; PAPER.md:95 step (5))
-        if (lane == 0) {
+        // (all lanes converged: every lane polls, fences and waits; one elected lane issues the TMA)
+        {
             uint32_t stage = 0, phase = 0;
             unsigned long long stall = 0, polls = 0;
             bool aborted = false;
@@ -792,10 +794,12 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 const uint32_t slot = it % kSchedSlots;
                 wait_shared(bar_sfull + 8 * slot, (it / kSchedSlots) & 1, pair);
                 const UnitInfo u = ring[slot];
-                arrive_leader(bar_sempty + 8 * slot, pair);
+                __syncwarp();  // every lane holds the unit before the slot is handed back
+                if (lane == 0) arrive_leader(bar_sempty + 8 * slot, pair);
                 if (!u.valid) break;
                 if (u.kind == kUnitReduce) continue;
                 const CUtensorMap* tm = &P.tm_a[u.layer];
+                const int a_row = P.m_off + u.m_blk * tile_m + (pair ? static_cast<int>(rank) * a_rows : 0);
                 const bool wait = P.wait_flags && u.layer > P.layer_begin && !u.acquired;
                 if (P.wait_flags && u.layer > P.layer_begin) fence_proxy_async();
                 const LayerParams& Lp = P.layer[u.layer > 0 ? u.layer - 1 : 0];
@@ -843,7 +847,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                                         if ((n & 255u) == 0) {
                                             if (ld_relaxed_gpu(P.status) != 0) { aborted = true; break; }
                                             if (globaltimer_ns() - t0 > P.timeout_ns) {
-                                                atomicCAS(P.status, 0u, kStatusFlagTimeout);
+                                                if (lane == 0) atomicCAS(P.status, 0u, kStatusFlagTimeout);
                                                 aborted = true;
                                                 break;
                                             }
@@ -862,18 +866,20 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                             pend_base = -1;
                         }
                     }
-                    if (pair) {  // each CTA stages HALF of the tokens (the B operand of the pair MMA is split between the CTAs)
-                        if (leader) mbar_arrive_expect_tx(bar_afull + 8 * stage, 2 * a_tile_bytes);
-                        tma_load_2d_pair(a_ring + stage * a_tile_bytes, tm, kb * kTileK, P.m_off + u.m_blk * tile_m + static_cast<int>(rank) * a_rows,
-                                         bar_afull + 8 * stage, pol_a);
-                    } else {
-                        mbar_arrive_expect_tx(bar_afull + 8 * stage, a_tile_bytes);
-                        tma_load_2d(a_ring + stage * a_tile_bytes, tm, kb * kTileK, P.m_off + u.m_blk * tile_m, bar_afull + 8 * stage);
+                    if (elect_one()) {
+                        if (pair) {  // each CTA stages HALF of the tokens (the B operand of the pair MMA is split between the CTAs)
+                            if (leader) mbar_arrive_expect_tx(bar_afull + 8 * stage, 2 * a_tile_bytes);
+                            tma_load_2d_pair(a_ring + stage * a_tile_bytes, tm, kb * kTileK, a_row, bar_afull + 8 * stage, pol_a);
+                        } else {
+                            mbar_arrive_expect_tx(bar_afull + 8 * stage, a_tile_bytes);
+                            tma_load_2d(a_ring + stage * a_tile_bytes, tm, kb * kTileK, a_row, bar_afull + 8 * stage);
+                        }
                     }
+                    __syncwarp();
                     if (++stage == static_cast<uint32_t>(a_stages)) { stage = 0; phase ^= 1; }
                 }
             }
-            if (!(P.flags & kFlagWorkQueue)) {
+            if (!(P.flags & kFlagWorkQueue) && lane == 0) {
                 P.stats[blockIdx.x].stall_cycles = stall;
                 P.stats[blockIdx.x].polls = polls;
             }
