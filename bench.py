@@ -27,6 +27,14 @@ if ROOT not in sys.path:
 METRIC = "mlp_2layer_gemm_latency_us"
 UNIT = "us"
 N_WEIGHT_SETS = 3  # rotating weight sets: no step can reuse the previous step's weights from L2
+L2_BYTES = 126e6
+
+
+def weight_sets_for(cfg):
+    """Rotating weight sets: at least 3, and enough of them that one full rotation is larger than twice the L2 (a small
+    config such as cfg 0 would otherwise be served from L2 step after step)."""
+    w_bytes = sum(2 * cfg.widths[l] * cfg.widths[l + 1] for l in range(cfg.n_layers))
+    return int(min(64, max(N_WEIGHT_SETS, -(-int(2 * L2_BYTES) // w_bytes))))
 
 
 def parse_args():
@@ -286,7 +294,8 @@ def main():
         cfg = inputs.Config("custom_" + "x".join(map(str, dims)), dims[0], tuple(dims[1:]), args.act if args.act >= 0 else 0, "normal", 7,
                             "custom shape (--shape)")
     mode = make_mode(B, args, cfg.n_layers)
-    X, sets = device_inputs(torch, cfg, N_WEIGHT_SETS)
+    n_sets = weight_sets_for(cfg)
+    X, sets = device_inputs(torch, cfg, n_sets)
     Y = torch.empty((cfg.M, cfg.widths[-1]), dtype=torch.bfloat16, device="cuda")
     pipe = B.MlpPipe(cfg.M, cfg.widths, cfg.act, mode)
     sampler = ClockSampler(nvml_index_for(torch, local))
@@ -326,10 +335,10 @@ def main():
         "dtype": "bf16 in/out, fp32 accumulate", "data": "synthetic",
         "config": {"workload": (f"custom: M={cfg.M} widths={list(cfg.widths)} act={cfg.act}" if args.shape else
                                 f"BASELINE.json configs[{args.config}]: {cfg.name} M={cfg.M} widths={list(cfg.widths)} act={cfg.act}"),
-                   "mode": args.mode, "cta_pairs": bool(args.pair), "grid": st.grid, "tile_m": st.tile_m, "stages": st.stages,
+                   "mode": args.mode, "chunks": args.chunks if args.mode == "microbatch" else None, "cta_pairs": bool(args.pair), "grid": st.grid, "tile_m": st.tile_m, "stages": st.stages,
                    "split_k": list(st.split_k)[:cfg.n_layers], "sm_split": args.sm_split, "tile_n": st.tile_n,
-                   "plan": "modelled" if args.no_autotune else "autotuned on the first warm-up run (MLP_FLAG_AUTOTUNE)",
-                   "l2": f"inputs larger than L2: {N_WEIGHT_SETS} rotating weight sets of {alg_bytes / 1e6:.0f} MB, no weight reuse across steps",
+                   "plan": "modelled" if (args.no_autotune or args.mode == "microbatch") else "autotuned on the first warm-up run (MLP_FLAG_AUTOTUNE)",
+                   "l2": f"inputs larger than L2: {n_sets} rotating weight sets of {alg_bytes / 1e6:.0f} MB, no weight reuse across steps",
                    "multi_gpu": "replicas only"},
         "latency_us": lat, "clocks": clocks, "gpu_launches": args.steps * launches_per_step, "roofline": roofline,
         "flag_stall_cycles_max": int(st.flag_stall_cycles_max),

@@ -39,7 +39,7 @@ def main() -> int:
     cfg = inputs.CONFIGS[args.config]
     kind = B.MLP_CTA_PIPELINED if args.mode == "pipelined" else B.MLP_SEQUENTIAL
     flags = (0 if args.no_autotune else B.MLP_FLAG_AUTOTUNE) | (B.MLP_FLAG_WORKQUEUE if args.workqueue else 0) | (B.MLP_FLAG_PAIR if args.pair else 0)
-    X, sets = bench.device_inputs(torch, cfg, bench.N_WEIGHT_SETS)
+    X, sets = bench.device_inputs(torch, cfg, bench.weight_sets_for(cfg))
     Y = torch.empty((cfg.M, cfg.widths[-1]), dtype=torch.bfloat16, device="cuda")
     p = B.MlpPipe(cfg.M, cfg.widths, cfg.act, B.make_mode(kind, flags=flags))
     lat, _ = bench.time_steps(torch, p, X, sets, Y, 50, 10)
