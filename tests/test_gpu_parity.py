@@ -457,12 +457,13 @@ PAIR = B.MLP_FLAG_PAIR
 
 @pytest.mark.parametrize("kw", [dict(kind=P), dict(kind=S), dict(kind=P, split_k=4), dict(kind=P, split_k_layer=[2, 8]), dict(kind=MB, chunks=2),
                                 dict(kind=P, flags=B.MLP_FLAG_DEBUG_DELAY, split_k=2), dict(kind=P, stages=2, a_stages=2), dict(kind=P, grid=2),
-                                dict(kind=P, flags=B.MLP_FLAG_AUTOTUNE)],
-                         ids=[str(i) for i in range(9)])
+                                dict(kind=P, flags=B.MLP_FLAG_AUTOTUNE), dict(kind=P, stages=3, a_stages=5, split_k=2)],
+                         ids=[str(i) for i in range(10)])
 def test_cta_pair_mode_exact(kw):
     """MLP_FLAG_PAIR (tcgen05 cta_group::2, clusters of two; SURVEY.md NEXT-3, PAPER.md:131-133): a pair executes a unit of
     256 weight rows, each CTA staging its 128 rows and half of the tokens; counters / partials / outputs stay per 128-row
-    block.  Exact-mode bits on cfg 0 and on ragged shapes (odd number of 128-row blocks, several M-blocks, 3 layers)."""
+    block.  Exact-mode bits on cfg 0 and on ragged shapes (odd number of 128-row blocks, several M-blocks, 3 layers).
+    (Case 9: rings of different depth = separate barriers per ring, two waits + two commits per K-block.)"""
     kw = dict(kw)
     kw["flags"] = kw.get("flags", 0) | PAIR
     check(inputs.get_config(0, "exact"), B.make_mode(**kw))
