@@ -48,6 +48,7 @@ def parse_args():
     ap.add_argument("--chunks", type=int, default=2)
     ap.add_argument("--sm-split", type=float, default=1.0)
     ap.add_argument("--stages", type=int, default=0)
+    ap.add_argument("--a-stages", type=int, default=0, help="activation ring depth (0 = library default)")
     ap.add_argument("--split-k", type=str, default="", help="comma list, per layer")
     ap.add_argument("--no-extras", action="store_true", help="skip the side measurements (other modes, e2e, cpu baseline)")
     ap.add_argument("--e2e-steps", type=int, default=5)
@@ -160,7 +161,7 @@ def make_mode(B, args, n_layers):
     kind = {"pipelined": B.MLP_CTA_PIPELINED, "sequential": B.MLP_SEQUENTIAL, "microbatch": B.MLP_MICROBATCH}[args.mode]
     split = [int(x) for x in args.split_k.split(",")] if args.split_k else []
     return B.make_mode(kind, chunks=args.chunks if kind == B.MLP_MICROBATCH else 0, sm_split=args.sm_split,
-                       stages=args.stages, split_k_layer=split,
+                       stages=args.stages, a_stages=args.a_stages, split_k_layer=split,
                        flags=(0 if args.no_autotune else B.MLP_FLAG_AUTOTUNE) | (B.MLP_FLAG_PAIR if args.pair else 0))
 
 

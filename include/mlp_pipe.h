@@ -135,8 +135,8 @@ typedef struct {
     int w_group;     /* weight K-blocks (128-byte row pieces) requested back to back: 0 = auto, <= stages   */
     int timeout_ms;  /* flag-poll watchdog: 0 = 2000 ms.  On expiry the kernel stops waiting, finishes
                         with undefined output and the handle reports MLP_ERR_TIMEOUT                   */
-    int a_stages;    /* activation ring depth: 0 = auto (activations come from L2, weights from HBM: the two
-                        rings need different depths for the same bandwidth)                             */
+    int a_stages;    /* activation ring depth: 0 = as deep as the weight ring (the two rings then share their
+                        barriers: one wait + one commit per K-block); another value gives the ring its own  */
 } mlp_mode;
 
 /*

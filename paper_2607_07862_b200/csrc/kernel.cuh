@@ -407,8 +407,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
     const uint32_t w_tile_bytes = static_cast<uint32_t>(n_sub) * kWTileBytes;
     const uint32_t a_tile_bytes = static_cast<uint32_t>(a_rows) * (kTileK * 2);
     const int stages = P.stages;      // weight ring depth
-    const int a_stages = P.a_stages;  // activation ring depth (its own, deeper ring: the consumer prologue's
-                                      // polls and fences then run K-blocks ahead of the weight stream)
+    const int a_stages = P.a_stages;  // activation ring depth (= stages unless mlp_mode.a_stages asks otherwise)
     // Equally deep rings share their barriers: "stage s landed" counts the bytes of both tiles (two arrivals, one per
     // loader), "stage s consumed" is ONE commit that both loaders wait for -- one wait and one commit per K-block.
     const bool unified = stages == a_stages;
