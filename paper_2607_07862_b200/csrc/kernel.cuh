@@ -28,7 +28,9 @@
 //                            prefetched up to the ring depth before A^l exists
 //     warp 2  A loader      consumer prologue: polls the (M-block, K-slice) ready counters (ld.relaxed.gpu + one
 //                            fence.acq_rel.gpu, or ld.acquire.gpu), then TMA-loads the activation tile [step a5]
-//     warp 3  MMA issuer    tcgen05.mma into TMEM; owns TMEM alloc / dealloc                [a2, a6]
+//                            (32 lanes converged, one elected lane issues the TMA)
+//     warp 3  MMA issuer    tcgen05.mma into TMEM (32 lanes converged, one elected lane issues: the issue loop paces
+//                            the tensor pipe, see the role); owns TMEM alloc / dealloc       [a2, a6]
 //     warps 4-7 epilogue    tcgen05.ld -> act -> bf16 -> transposed store, or fp32 split-K partial (+ gather by the
 //                            last arriver), or a reduce unit; then producer epilogue: fence + red.release.gpu
 //                            publish (+ scoreboard / queue push in work-queue mode)          [a3, a4, a7, a8]
