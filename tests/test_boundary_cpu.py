@@ -51,6 +51,33 @@ def test_sass_is_blackwell_native():
     assert "HMMA." not in sass.replace("UTCHMMA", ""), "legacy mma.sync path must not be present"
 
 
+def test_mma_issue_loop_has_no_per_instruction_elect_loops():
+    """The MMA warp runs converged and issues under elect.sync ("The MMA issuer paces the tensor pipe"): every
+    UTCHMMA of the kernel must be straight-line code.  A `lane == 0` thread would make ptxas wrap each one into an ELECT / BRA.U.ANY
+    loop over the active lanes, which is what paced the tensor pipe before."""
+    from paper_2607_07862_b200 import build
+
+    cuobjdump = "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(cuobjdump):
+        pytest.skip("cuobjdump not installed")
+    sass = subprocess.run([cuobjdump, "-sass", build.build_lib()], capture_output=True, text=True).stdout
+    lines = [l for l in sass.splitlines() if re.search(r"/\*[0-9a-f]{4,}\*/\s+\S", l)]
+    mma = [i for i, l in enumerate(lines) if "UTCHMMA" in l]
+    assert mma, "no tcgen05.mma in the library"
+    for i in mma:
+        window = " ".join(lines[i + 1:i + 4])
+        assert "BRA.U.ANY" not in window, "UTCHMMA inside an elect loop:\n" + "\n".join(lines[i - 2:i + 4])
+
+
+def test_mma_issue_microbenchmark_compiles(tmp_path):
+    """csrc/bench_mma_issue.cu (developer microbenchmark behind profiles/r1d_mma_issue_microbench.txt) still builds for sm_100a."""
+    nvcc = "/usr/local/cuda/bin/nvcc"
+    if not os.path.exists(nvcc):
+        pytest.skip("nvcc not installed")
+    src = os.path.join(ROOT, "paper_2607_07862_b200", "csrc", "bench_mma_issue.cu")
+    subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-c", src, "-o", str(tmp_path / "b.o")], check=True)
+
+
 def test_header_compiles_as_plain_c(tmp_path):
     src = tmp_path / "t.c"
     src.write_text('#include "mlp_pipe.h"\nint main(void){ mlp_mode m = {0}; mlp_stats s; mlp_cta_record r; (void)m; (void)s; (void)r; '

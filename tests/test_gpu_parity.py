@@ -544,3 +544,24 @@ def test_paper_shape_sampled_rows():
         assert st.status == 0 and st.ready_ok == 1
         e = oracle.rel_err(got[rows], outs[-1])
         assert e["nan"] == 0 and e["err"] <= TOL, e
+
+
+def test_bench_custom_shape_line_is_well_formed():
+    """`bench.py --shape ... --pair` (the command behind profiles/paper_workload_r1d.md) on a small chain: one JSON line with the
+    contract's keys, a tensor- or HBM-bound roofline object and the in-build launch count."""
+    import json
+    import os
+    import subprocess
+    import sys
+
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--shape", "512,1024,1024,1024", "--act", "0", "--pair", "--no-extras",
+                          "--no-autotune", "--steps", "5", "--warmup", "3"], capture_output=True, text=True, timeout=600, cwd=root)
+    assert out.returncode == 0, out.stderr[-2000:]
+    line = json.loads(out.stdout.strip().splitlines()[-1])
+    for key in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling", "vs_baseline", "dtype",
+                "data", "config", "clocks", "gpu_launches", "roofline"):
+        assert key in line, key
+    assert line["config"]["cta_pairs"] is True and line["config"]["workload"].startswith("custom: M=512")
+    assert line["roofline"]["bound"] in ("tensor", "hbm") and 0 < line["roofline"]["frac"] < 1.5
+    assert line["gpu_launches"] == 5 and line["value"] > 0
