@@ -25,7 +25,7 @@
 //     warp 0  scheduler     global atomic ticket -> unit table -> smem ring (broadcast), drawn late; fast-path look
 //                            at the unit's ready counters; in work-queue mode: pops the unit from the queue  [step a1]
 //     warp 1  W loader      TMA loads of weight tiles; never waits on a flag, so W_{l+1} is
-//                            prefetched up to the ring depth before A^l exists
+//                            prefetched up to the ring depth before A^l exists (32 lanes converged, one elected issuer)
 //     warp 2  A loader      consumer prologue: polls the (M-block, K-slice) ready counters (ld.relaxed.gpu + one
 //                            fence.acq_rel.gpu, or ld.acquire.gpu), then TMA-loads the activation tile [step a5]
 //                            (32 lanes converged, one elected lane issues the TMA)
@@ -707,34 +707,39 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
             }
         }
     } else if (warp == 1) {
-        // ===== W loader (one thread: measured, the converged form of the other roles is SLOWER here -- paper workload with
-        // pairs 1487 vs 1445 us, cfg 1 55.6 vs 53.4 us)
-        if (lane == 0) {
+        // ===== W loader: all 32 lanes run the loop converged and wait, one elected lane issues.  (Measured: what makes a
+        // converged role slow is divergence INSIDE its loop -- a probe-then-wait branch per stage, `if (lane == 0)` arrivals,
+        // or worst of all one lane waiting while the others sit at a __syncwarp (cfg 1 66 instead of 51 us); with plain waits
+        // and every single-lane action under elect.sync it beats the one-thread form: cfg 1 mean 50.7 vs 51.4 us.)
+        {
             const uint64_t pol = policy_evict_first();
             const bool hint = !(P.flags & kFlagNoEvictFirst);
             uint32_t stage = 0, phase = 0;
-            unsigned long long w_wait = 0;
+            unsigned long long w_wait = 0;  // cycles inside the waits for a free stage (a wait that succeeds at once costs ~100)
             for (uint32_t it = 0;; ++it) {
                 const uint32_t slot = it % kSchedSlots;
                 wait_shared(bar_sfull + 8 * slot, (it / kSchedSlots) & 1, pair);
                 const UnitInfo u = ring[slot];
-                arrive_leader(bar_sempty + 8 * slot, pair);
+                __syncwarp();  // every lane holds the unit before the slot is handed back
                 // Late binding: the scheduler may draw the NEXT ticket only once this unit has at most
                 // claim_ahead K-blocks left to request.  A unit stalled on its producers (the ring is full, the
                 // MMA warp waits for the activation loader) therefore never holds a second ticket.
                 // (For a reduce unit the epilogue warps give the go once its partials have arrived.)
                 bool told = u.kind == kUnitReduce || !u.valid || u.kb1 - u.kb0 <= P.claim_ahead;
-                if (told && u.kind != kUnitReduce) mbar_arrive(bar_wtaken + 8 * slot);
+                if (elect_one()) {
+                    arrive_leader(bar_sempty + 8 * slot, pair);
+                    if (told && u.kind != kUnitReduce) mbar_arrive(bar_wtaken + 8 * slot);
+                    if (u.valid && it < kUnitTrace) {
+                        const uint64_t now = globaltimer_ns();
+                        my_stats->unit_ts[it][0] = now;
+                        if (u.kind == kUnitReduce) my_stats->unit_ts[it][1] = now;
+                        my_stats->unit_id[it] = (static_cast<uint32_t>(u.layer) << 28) | (static_cast<uint32_t>(u.tile) << 8) |
+                                                static_cast<uint32_t>(u.kind == kUnitReduce ? 0x80 | (u.kb0 >> 4) : u.ks);
+                    }
+                }
+                __syncwarp();
                 if (!u.valid) break;
-                if (it < kUnitTrace) {
-                    my_stats->unit_ts[it][0] = globaltimer_ns();
-                    my_stats->unit_id[it] = (static_cast<uint32_t>(u.layer) << 28) | (static_cast<uint32_t>(u.tile) << 8) |
-                                            static_cast<uint32_t>(u.kind == kUnitReduce ? 0x80 | (u.kb0 >> 4) : u.ks);
-                }
-                if (u.kind == kUnitReduce) {
-                    if (it < kUnitTrace) my_stats->unit_ts[it][1] = my_stats->unit_ts[it][0];
-                    continue;
-                }
+                if (u.kind == kUnitReduce) continue;
                 const CUtensorMap* tm = &P.tm_w[u.layer];
                 // K-blocks are requested in groups of w_group: the loader first waits until the whole group of
                 // stages is free and then issues the group back to back, so that the 128-byte pieces of one
@@ -746,35 +751,41 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                     stage = pre % static_cast<uint32_t>(stages);
                     phase = pre / static_cast<uint32_t>(stages);
                 }
+                const int w_row = pair ? (u.n_blk * 2 + static_cast<int>(rank)) * kTileN : u.n_blk * tile_n;
                 while (kb < u.kb1) {
                     const int g = min(P.w_group, u.kb1 - kb);
                     uint32_t st = stage, ph = phase;
+                    const long long t0 = clock64();
                     for (int i = 0; i < g; ++i) {
-                        mbar_wait_timed(bar_empty + 8 * st, ph ^ 1, w_wait);
+                        mbar_wait(bar_empty + 8 * st, ph ^ 1);
                         if (++st == static_cast<uint32_t>(stages)) { st = 0; ph ^= 1; }
                     }
-                    if (!told && u.kb1 - kb <= P.claim_ahead) {
-                        told = true;
-                        mbar_arrive(bar_wtaken + 8 * slot);
-                    }
+                    w_wait += static_cast<unsigned long long>(clock64() - t0);
+                    const bool tell = !told && u.kb1 - kb <= P.claim_ahead;
+                    told = told || tell;
                     for (int i = 0; i < g; ++i, ++kb) {
                         const uint32_t full = bar_full + 8 * stage;
                         const uint32_t dst = smem_base + stage * w_tile_bytes;
-                        if (pair) {
-                            // each CTA loads its own 128 weight rows; the bytes of BOTH count on the leader's barrier
-                            if (leader) mbar_arrive_expect_tx(full, 2 * w_tile_bytes);
-                            tma_load_2d_pair(dst, tm, kb * kTileK, (u.n_blk * 2 + static_cast<int>(rank)) * kTileN, full, pol);
-                        } else {
-                            mbar_arrive_expect_tx(full, w_tile_bytes);
-                            if (hint) tma_load_2d_hint(dst, tm, kb * kTileK, u.n_blk * tile_n, full, pol);
-                            else tma_load_2d(dst, tm, kb * kTileK, u.n_blk * tile_n, full);
+                        if (elect_one()) {
+                            if (tell && i == 0) mbar_arrive(bar_wtaken + 8 * slot);
+                            if (pair) {
+                                // each CTA loads its own 128 weight rows; the bytes of BOTH count on the leader's barrier
+                                if (leader) mbar_arrive_expect_tx(full, 2 * w_tile_bytes);
+                                tma_load_2d_pair(dst, tm, kb * kTileK, w_row, full, pol);
+                            } else {
+                                mbar_arrive_expect_tx(full, w_tile_bytes);
+                                if (hint) tma_load_2d_hint(dst, tm, kb * kTileK, w_row, full, pol);
+                                else tma_load_2d(dst, tm, kb * kTileK, w_row, full);
+                            }
                         }
+                        __syncwarp();
                         if (++stage == static_cast<uint32_t>(stages)) { stage = 0; phase ^= 1; }
                     }
                 }
-                if (it < kUnitTrace) my_stats->unit_ts[it][1] = globaltimer_ns();
+                if (it < kUnitTrace && elect_one()) my_stats->unit_ts[it][1] = globaltimer_ns();
+                __syncwarp();
             }
-            my_stats->wait[0] = w_wait;
+            if (lane == 0) my_stats->wait[0] = w_wait;
         }
     } else if (warp == 2) {
         // ===== A loader = consumer prologue (step a5; PAPER.md:95 step (5))
