@@ -228,7 +228,8 @@ typedef struct {
     uint64_t ts[8];               /* globaltimer ns: 0 CTA start, 1 setup done, 2 first ticket decoded,
                                      3 first weight TMA issued, 4 first stage landed, 5 first accumulator
                                      complete, 6 first unit stored (+published), 7 CTA exit               */
-    uint64_t wait[8];             /* SM cycles: 0 weight loader blocked on a free stage, 1 reducer summing
+    uint64_t wait[8];             /* SM cycles: 0 weight loader inside its waits for a free stage (every wait is timed: one
+                                     that succeeds at once still costs ~100 cycles per K-block), 1 reducer summing
                                      partials (gather loads + adds), 2 MMA blocked on operands, 3 MMA blocked
                                      on a free accumulator, 4 epilogue blocked on an accumulator, 5 reduce unit
                                      blocked on the arrival counter of its tile, 6 storing split-K partials,
