@@ -330,6 +330,9 @@ def main():
                     "peak_source": "measured (MEASURED_PEAKS.json bf16_tflops_sustained)" if mp else "fallback (B200_PROFILING.md 1.59 PFLOP/s)",
                     "kernel": "mlp_pipe_kernel", "flops_per_step": cfg.flops, "avg_step_us": lat["mean"],
                     "roofline_us_at_peak": cfg.flops / (tpeak * 1e6), "tflops": cfg.flops / value / 1e6}
+    # BASELINE.json's own roofline: max(FLOPs / dense-bf16 datasheet peak, bytes / ~8 TB/s) -- context beside the measured peaks
+    nominal_us = max(cfg.flops / (2250.0 * 1e6), alg_bytes / 8000.0 / 1e3)
+    roofline["nominal"] = {"tensor_tflops": 2250.0, "hbm_gbs": 8000.0, "roofline_us": nominal_us, "frac": nominal_us / lat["mean"]}
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
