@@ -564,4 +564,7 @@ def test_bench_custom_shape_line_is_well_formed():
         assert key in line, key
     assert line["config"]["cta_pairs"] is True and line["config"]["workload"].startswith("custom: M=512")
     assert line["roofline"]["bound"] in ("tensor", "hbm") and 0 < line["roofline"]["frac"] < 1.5
+    nominal = line["roofline"]["nominal"]  # BASELINE.json's formula with the datasheet peaks, beside the measured-peak fraction
+    flops, nbytes = 2 * 512 * 1024 * 1024 * 2, 2 * (512 * 1024 * 4 + 2 * 1024 * 1024)  # X, H written + read, Y; two weights
+    assert abs(nominal["roofline_us"] - max(flops / 2250e6, nbytes / 8e6)) < 1e-6 and 0 < nominal["frac"] < 1.5
     assert line["gpu_launches"] == 5 and line["value"] > 0
