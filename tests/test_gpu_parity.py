@@ -88,6 +88,8 @@ TINY = [
     # (M, widths, act): single tile / single k-block / ragged tails in every dimension
     (16, (64, 128, 128), 1), (1, (8, 8, 8), 1), (7, (72, 136, 8), 0), (50, (200, 328, 136), 2),
     (130, (264, 392, 200), 1), (300, (136, 264, 136), 1), (16, (64, 128, 128, 128), 1),
+    # the ends of the chain length: a single GEMM (L = 1, nothing to pipeline) and MLP_MAX_LAYERS = 8 linked layers
+    (40, (136, 200), 1), (24, (64, 128, 72, 136, 64, 128, 64, 200, 64), 2),
 ]
 
 
@@ -95,7 +97,7 @@ TINY = [
 @pytest.mark.parametrize("kind", [S, P])
 def test_edge_shapes_exact(M, widths, act, kind):
     """empty-ish and ragged shapes: M = 1, M not a multiple of 16, N / K not multiples of the tile, M > 256
-    (several M-blocks), 3 layers.  Integer inputs -> bit-exact (act NONE / RELU) or within tolerance (GeLU)."""
+    (several M-blocks), 1 / 3 / 8 layers.  Integer inputs -> bit-exact (act NONE / RELU) or within tolerance (GeLU)."""
     dist = "exact" if act != 2 else "normal"
     cfg = inputs.Config(f"edge_{M}_{'_'.join(map(str, widths))}", M, widths, act, dist, 11)
     check(cfg, B.make_mode(kind, split_k=2))
