@@ -10,7 +10,7 @@ S, MB, P = B.MLP_SEQUENTIAL, B.MLP_MICROBATCH, B.MLP_CTA_PIPELINED
 
 SHAPES = [(c.M, tuple(c.widths)) for c in inputs.CONFIGS] + [
     (1, (8, 8, 8)), (7, (72, 136, 8)), (300, (136, 264, 136)), (130, (264, 392, 200)), (16, (64, 128, 128, 128)),
-    (1024, (8192, 8192, 8192)),
+    (1024, (8192, 8192, 8192)), (40, (136, 200)), (24, (64, 128, 72, 136, 64, 128, 64, 200, 64)),  # L = 1 and L = MLP_MAX_LAYERS
 ]
 MODES = [
     dict(kind=P), dict(kind=S), dict(kind=MB, chunks=1), dict(kind=P, sm_split=0.5), dict(kind=P, split_k=4),
