@@ -70,6 +70,7 @@ struct UnitDesc {
 static_assert(sizeof(UnitDesc) == 8, "UnitDesc is read as one 8-byte word");
 
 constexpr int kActNone = 0, kActRelu = 1, kActGeluTanh = 2;
+constexpr float kGelu0 = 0.7978845608028654f, kGelu1 = 0.7978845608028654f * 0.044715f;  // sqrt(2/pi), sqrt(2/pi) * 0.044715
 constexpr uint32_t kFlagTileMajor = 0x1u, kFlagDebugDelay = 0x2u, kFlagDebugReverse = 0x4u, kFlagNoEvictFirst = 0x8u;
 // measurement knobs (include/mlp_pipe.h MLP_FLAG_EXP_*): each removes or replaces one protocol ingredient
 constexpr uint32_t kFlagExpNoAcquireFence = 0x10u, kFlagExpNoProxyFence = 0x20u, kFlagAcquireLoads = 0x40u,
@@ -163,12 +164,40 @@ template <int act>
 __device__ __forceinline__ float act_apply(float x) {
     if (act == kActRelu) return x > 0.0f ? x : 0.0f;
     if (act == kActGeluTanh) {
-        float u = 0.7978845608028654f * (x + 0.044715f * x * x * x);
+        // g(x) = 0.5 x (1 + tanh(sqrt(2/pi) (x + 0.044715 x^3))) as mul, fma, mul, MUFU, mul, fma; kGelu1 = sqrt(2/pi) * 0.044715
+        const float u = x * fmaf(x * x, kGelu1, kGelu0);
         float t;
         asm("tanh.approx.f32 %0, %1;" : "=f"(t) : "f"(u));
-        return 0.5f * x * (1.0f + t);
+        const float hx = 0.5f * x;
+        return fmaf(hx, t, hx);
     }
     return x;
+}
+
+// Two GeLUs at once on the packed fp32 pipe (mul.f32x2 / fma.rn.f32x2: one issue slot per pair), the same operations in
+// the same order as act_apply<kActGeluTanh> lane by lane, so the result is bit-identical to it: the epilogue warps (one
+// per sub-partition) are issue-bound at large token tiles, and the arithmetic of the activation is most of their slots.
+__device__ __forceinline__ void gelu_tanh_x2(float xa, float xb, float& ya, float& yb) {
+    uint64_t x, c0, c1, h, u, t, y;
+    float ua, ub, ta, tb;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(x) : "f"(xa), "f"(xb));
+    asm("mov.b64 %0, {%1, %1};" : "=l"(c0) : "f"(kGelu0));
+    asm("mov.b64 %0, {%1, %1};" : "=l"(c1) : "f"(kGelu1));
+    asm("mov.b64 %0, {%1, %1};" : "=l"(h) : "f"(0.5f));
+    asm("{\n\t.reg .b64 x2, p;\n\t"
+        "mul.f32x2 x2, %1, %1;\n\t"
+        "fma.rn.f32x2 p, x2, %2, %3;\n\t"
+        "mul.f32x2 %0, %1, p;\n\t}"
+        : "=l"(u) : "l"(x), "l"(c1), "l"(c0));
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(ua), "=f"(ub) : "l"(u));
+    asm("tanh.approx.f32 %0, %1;" : "=f"(ta) : "f"(ua));
+    asm("tanh.approx.f32 %0, %1;" : "=f"(tb) : "f"(ub));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(t) : "f"(ta), "f"(tb));
+    asm("{\n\t.reg .b64 hx;\n\t"
+        "mul.f32x2 hx, %1, %2;\n\t"
+        "fma.rn.f32x2 %0, hx, %3, hx;\n\t}"
+        : "=l"(y) : "l"(x), "l"(h), "l"(t));
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(ya), "=f"(yb) : "l"(y));
 }
 
 __device__ __forceinline__ float ld_cg_f32(const float* p) {
@@ -216,9 +245,19 @@ template <int kCols, int kAct>
 __device__ __forceinline__ void stage_cols(const uint32_t (&f)[kCols], uint32_t buf, int r) {
     // the activation is a compile-time choice here: a run-time switch per element would serialise the
     // 32 independent columns behind one another's MUFU latency
+    if constexpr (kAct == kActGeluTanh) {
 #pragma unroll
-    for (int j = 0; j < kCols; ++j)
-        st_shared_b16(buf + static_cast<uint32_t>(j * kTileN + r) * 2u, __bfloat16_as_ushort(__float2bfloat16_rn(act_apply<kAct>(__uint_as_float(f[j])))));
+        for (int j = 0; j < kCols; j += 2) {
+            float ya, yb;
+            gelu_tanh_x2(__uint_as_float(f[j]), __uint_as_float(f[j + 1]), ya, yb);
+            st_shared_b16(buf + static_cast<uint32_t>(j * kTileN + r) * 2u, __bfloat16_as_ushort(__float2bfloat16_rn(ya)));
+            st_shared_b16(buf + static_cast<uint32_t>((j + 1) * kTileN + r) * 2u, __bfloat16_as_ushort(__float2bfloat16_rn(yb)));
+        }
+    } else {
+#pragma unroll
+        for (int j = 0; j < kCols; ++j)
+            st_shared_b16(buf + static_cast<uint32_t>(j * kTileN + r) * 2u, __bfloat16_as_ushort(__float2bfloat16_rn(act_apply<kAct>(__uint_as_float(f[j])))));
+    }
 }
 
 template <int kCols>
