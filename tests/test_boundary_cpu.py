@@ -49,6 +49,9 @@ def test_sass_is_blackwell_native():
     for mnemonic in ["UTCHMMA", "LDTM", "UTMALDG", "REDG.E.ADD.STRONG.GPU", "LDG.E.STRONG.GPU"]:
         assert mnemonic in sass, mnemonic
     assert "HMMA." not in sass.replace("UTCHMMA", ""), "legacy mma.sync path must not be present"
+    # the GeLU epilogue runs on the packed fp32 pipe: 5 packed operations per 2 tanh (cfg 2 anatomy)
+    packed, tanh = len(re.findall(r"\b(?:FMUL2|FFMA2)\b", sass)), sass.count("MUFU.TANH")
+    assert tanh > 0 and packed * 2 == tanh * 5, (packed, tanh)
 
 
 def test_mma_issue_loop_has_no_per_instruction_elect_loops():
