@@ -39,6 +39,12 @@
  *     H_l, tickets, counters, the split-K workspace, tensor maps and internal streams.
  *   - a handle is NOT re-entrant: runs on one handle must be stream-ordered after one
  *     another (all counters are per handle).
+ *   - co-residency: a persistent launch needs all its CTAs (<= one per SM) on the device at the
+ *     same time, because waiting CTAs wait on work owned by other CTAs of the launch.  Launches
+ *     that can wait are therefore cooperative (they queue behind other work instead of starting
+ *     partially); see MLP_FLAG_NO_COOPERATIVE.
+ *   - limits: ceil(N_l / 128) * ceil(M / tile_m) <= 65535 output tiles and K_l <= 64 * 65535 per
+ *     layer (MLP_ERR_UNSUPPORTED beyond).
  *   - there is no CPU fallback: without an sm_100 device mlp_pipe_create fails with
  *     MLP_ERR_UNSUPPORTED.
  */
@@ -107,13 +113,35 @@ enum {
                                        M = 256 for both tensor cores; counters, partials and outputs stay per 128-row block.
                                        Halves the activation bytes an SM pulls per weight byte.  tile_m must be a multiple of
                                        32 (UNSUPPORTED otherwise), grid even, not with MLP_FLAG_WORKQUEUE.                      */
+#define MLP_FLAG_DEBUG_DROP_PUBLISH 0x4000u /* test hook: the producer of output tile 0 of the first layer never publishes its
+                                       ready counter, so its consumers starve until the flag-poll watchdog (timeout_ms) expires:
+                                       the deterministic way to exercise MLP_ERR_TIMEOUT.  One-shot: only the FIRST run of the
+                                       handle drops the publish, so the runs after the reset are clean                            */
+#define MLP_FLAG_NO_COOPERATIVE 0x8000u /* launch WITHOUT cudaLaunchAttributeCooperative.  By default every launch in which a CTA
+                                       may wait on another CTA (CTA_PIPELINED; split-K reduce units in any mode) is cooperative:
+                                       the grid starts only when all its CTAs fit on the device at once.  With this flag the
+                                       caller guarantees that (an otherwise idle GPU, no second handle running concurrently);
+                                       otherwise waiting CTAs can starve CTAs that are not yet resident until the watchdog.   */
+#define MLP_FLAG_MB_CORESIDENT 0x10000u /* MICROBATCH only: every launch gets num_SMs / min(L, chunks) CTAs instead of one per SM, so
+                                       that the launches of different layers on their different streams fit on the device
+                                       TOGETHER and layer l of chunk i+1 really overlaps layer l+1 of chunk i (PAPER.md:173,
+                                       Fig. 3a).  Without it every launch is a full persistent grid that holds all SMs (shared
+                                       memory allows one CTA per SM), and the second stream only gets SMs as the first's CTAs exit. */
+#define MLP_FLAG_TWO_KERNEL 0x20000u /* CTA_PIPELINED, 2 layers: the paper's host organisation on one GPU (
+                                       SURVEY.md NEXT-4).  The producer layer is a kernel of its own on an internal stream over
+                                       sm_split x num_SMs CTAs (0 or 1 = one half), the consumer layer a second kernel on a
+                                       second stream over the remaining SMs, gated by cuStreamWaitValue32 on the first ready
+                                       counter reaching this run's value; inside the consumer kernel every unit polls its ready
+                                       counters as usual.  Not capturable into a CUDA graph (the wait value is per run), not
+                                       with MLP_FLAG_WORKQUEUE / PAIR / AUTOTUNE (UNSUPPORTED).                                 */
 #define MLP_FLAG_AUTOTUNE 0x400u    /* measured plan search: the FIRST mlp_pipe_run on the handle (outside stream
                                        capture) tries the planner's candidate K-splits / ticket orders (and, unless tile_n is given,
                                        both unit heights 128 / 256) on the
                                        caller's buffers, timing each with the in-kernel clock, and keeps the
                                        fastest.  That one call synchronises the device, may allocate, and takes
                                        tens of milliseconds; Y is valid after it.  Results are remembered per
-                                       process for equal (shape, mode).  SEQUENTIAL and CTA_PIPELINED only.  If the
+                                       process for equal (shape, mode).  MICROBATCH candidates are timed from fork to join
+                                       with CUDA events (its launches overlap).  If the
                                        first run is being captured into a CUDA graph the search is skipped for good. */
 
 typedef struct {
@@ -162,7 +190,10 @@ int mlp_pipe_create_chain(mlp_pipe** out, int M, int n_layers, const int* widths
  * a cudaStream_t (NULL = the legacy default stream).  Asynchronous: enqueues on the stream
  * and returns; no host synchronisation, no allocation.  Y is fully overwritten.
  * Errors: INVALID (null / misaligned pointer), CUDA (launch failure, see last_error),
- * TIMEOUT (a previous run on this handle hit the watchdog; the handle has been reset).
+ * TIMEOUT (a previous run on this handle hit the watchdog: the kernel mirrors its status word into
+ * pinned host memory, so the first mlp_pipe_run AFTER the expired kernel has finished sees it without
+ * a device round trip, synchronises, resets the handle's protocol state and returns TIMEOUT once; the
+ * output of the expired run, and of runs that were already queued behind it, is undefined).
  */
 int mlp_pipe_run(mlp_pipe* h, const void* X, const void* W1, const void* W2, void* Y, void* cuda_stream);
 

@@ -25,6 +25,10 @@ MLP_FLAG_AUTOTUNE = 0x400
 MLP_FLAG_PDL = 0x800
 MLP_FLAG_WORKQUEUE = 0x1000
 MLP_FLAG_PAIR = 0x2000
+MLP_FLAG_DEBUG_DROP_PUBLISH = 0x4000
+MLP_FLAG_NO_COOPERATIVE = 0x8000
+MLP_FLAG_MB_CORESIDENT = 0x10000
+MLP_FLAG_TWO_KERNEL = 0x20000
 MLP_FLAG_ACQUIRE_LOADS, MLP_FLAG_EXP_NO_ACQUIRE_FENCE, MLP_FLAG_EXP_NO_PROXY_FENCE = 0x40, 0x10, 0x20
 MLP_FLAG_EXP_NO_FAST_PATH, MLP_FLAG_EXP_NO_PREISSUE = 0x80, 0x100
 

@@ -44,7 +44,9 @@ def build_lib(force: bool = False, verbose: bool = False) -> str:
     """Compile the C-ABI library if it is missing or older than its sources; return its path."""
     if not force and not needs_build():
         return LIB
-    cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SOURCES
+    # MLP_PIPE_DEBUG_HOOKS=1: developer build whose planner reads MLP_PIPE_BOUNDS_<l> / MLP_PIPE_NO_RASTER / MLP_PIPE_DEBUG
+    hooks = ["-DMLP_PIPE_DEBUG_HOOKS"] if os.environ.get("MLP_PIPE_DEBUG_HOOKS") == "1" else []
+    cmd = [_nvcc()] + NVCC_FLAGS + hooks + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SOURCES
     res = subprocess.run(cmd, cwd=CSRC, capture_output=True, text=True)
     if verbose:
         sys.stderr.write(res.stdout + res.stderr)

@@ -77,6 +77,7 @@ constexpr uint32_t kFlagExpNoAcquireFence = 0x10u, kFlagExpNoProxyFence = 0x20u,
                    kFlagExpNoFastPath = 0x80u, kFlagExpNoPreissue = 0x100u;
 constexpr uint32_t kFlagWorkQueue = 0x1000u;  // consumers pop ready units from a work queue instead of polling ready counters
 constexpr uint32_t kFlagPdl = 0x800u;  // SEQUENTIAL: layer l+1 is launched as a programmatic dependent of layer l
+constexpr uint32_t kFlagDebugDropPublish = 0x4000u;  // test hook: the producer of tile 0 of the launch's first layer never publishes
 constexpr uint32_t kStatusFlagTimeout = 1u;
 
 struct LayerParams {
@@ -145,10 +146,13 @@ struct KernelParams {
     int wait_flags;     // consumer prologue on/off
     int pair;           // 1: CTA pairs (cluster of 2, tcgen05 cta_group::2): a pair executes one unit of 256 weight rows, each
                         // CTA loading its 128 rows and HALF of the activation tile; the leader (rank 0) schedules and issues
+    int wait_first;     // 1: the launch's FIRST layer is a consumer too -- its producer runs in another launch on another
+                        // stream (MLP_FLAG_TWO_KERNEL) and publishes the same ready counters
     int pdl_wait;       // 1: launched as a programmatic dependent; the activation loader waits for the grid before
     uint32_t flags;
     unsigned long long* epoch_counter;  // += 1 per exiting CTA; epoch = value / gridDim.x
     uint32_t* status;
+    uint32_t* status_host;  // the same word mirrored in pinned host memory (written on expiry only): mlp_pipe_run reads it for free
     unsigned long long timeout_ns;
     CtaStats* stats;
 };
@@ -394,10 +398,19 @@ __device__ __forceinline__ uint2 unit_words(const LayerParams& L, uint32_t t, bo
     return __ldg(reinterpret_cast<const uint2*>(L.table) + t);
 }
 
+// Watchdog expiry: record it in the device status word (every other waiter then gives up after its next 256 polls) and in
+// the pinned host mirror, where the next mlp_pipe_run on the handle finds it without a device round trip.
+__device__ __forceinline__ void flag_timeout(uint32_t* status, uint32_t* status_host) {
+    if (atomicCAS(status, 0u, kStatusFlagTimeout) == 0u && status_host) {
+        *reinterpret_cast<volatile uint32_t*>(status_host) = kStatusFlagTimeout;
+        __threadfence_system();
+    }
+}
+
 // Spin until *ctr has reached `target` (wrap-safe), then acquire.  Relaxed polls + one acquire fence =
 // acquire pattern.  Bounded: after timeout_ns (or when another waiter has already given up) the wait is
 // abandoned, the device status word records it and the caller carries on (output undefined, kernel ends).
-__device__ __forceinline__ void poll_counter(const uint32_t* ctr, uint32_t target, uint32_t* status,
+__device__ __forceinline__ void poll_counter(const uint32_t* ctr, uint32_t target, uint32_t* status, uint32_t* status_host,
                                              unsigned long long timeout_ns, unsigned long long& waited) {
     if (static_cast<int32_t>(ld_relaxed_gpu(ctr) - target) < 0) {
         const long long c0 = clock64();
@@ -408,7 +421,7 @@ __device__ __forceinline__ void poll_counter(const uint32_t* ctr, uint32_t targe
             if ((++n & 255u) == 0) {
                 if (ld_relaxed_gpu(status) != 0) break;
                 if (globaltimer_ns() - t0 > timeout_ns) {
-                    atomicCAS(status, 0u, kStatusFlagTimeout);
+                    flag_timeout(status, status_host);
                     break;
                 }
             }
@@ -546,7 +559,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                     tma_load_2d_hint(smem_base + i * w_tile_bytes, &P.tm_w[l0], (kb0 + static_cast<int>(i)) * kTileK, n_blk * tile_n, bar_full + 8 * i, pol);
                 else tma_load_2d(smem_base + i * w_tile_bytes, &P.tm_w[l0], (kb0 + static_cast<int>(i)) * kTileK, n_blk * tile_n, bar_full + 8 * i);
             }
-            if (l0 == P.layer_begin && !P.pdl_wait) {  // input of the launch: nothing to wait for
+            if (l0 == P.layer_begin && !P.pdl_wait && !P.wait_first) {  // input of the launch: nothing to wait for
                 pre_a = static_cast<uint32_t>(min(min(a_stages, stages), kb1 - kb0));
                 for (uint32_t i = 0; i < pre_a; ++i) {
                     mbar_arrive_expect_tx(bar_afull + 8 * i, a_tile_bytes);
@@ -627,6 +640,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 while (l < P.layer_end) {
                     const LayerParams& L = P.layer[l];
                     uint32_t t;
+                    const bool is_static = use_static;  // only the static ticket lies in the prefix the host verified against the closed form
                     if (use_static) {
                         use_static = false;
                         t = static_id;
@@ -658,7 +672,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                                 if ((++n & 255u) == 0) {
                                     if (ld_relaxed_gpu(P.status) != 0) { gave_up = true; break; }
                                     if (globaltimer_ns() - t0 > P.timeout_ns) {
-                                        atomicCAS(P.status, 0u, kStatusFlagTimeout);
+                                        flag_timeout(P.status, P.status_host);
                                         gave_up = true;
                                         break;
                                     }
@@ -672,7 +686,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                         raw = __ldg(reinterpret_cast<const uint2*>(L.table) + (v & 0xffffu));
                         popped = true;
                     } else {
-                        raw = unit_words(L, t, it == 0);
+                        raw = unit_words(L, t, is_static);
                     }
                     u.layer = l;
                     u.tile = static_cast<int>(raw.x & 0xffffu);
@@ -694,7 +708,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                             fence_acq_rel_gpu();
                             u.acquired = 1;
                         }
-                    } else if (P.wait_flags && l > P.layer_begin && !(P.flags & (kFlagExpNoFastPath | kFlagAcquireLoads))) {
+                    } else if (P.wait_flags && (l > P.layer_begin || P.wait_first) && !(P.flags & (kFlagExpNoFastPath | kFlagAcquireLoads))) {
                         // Consumer prologue, fast path (the prologue lives in the scheduler
                         // warp): one look at all ready counters under this unit's K range.  If every producer
                         // tile is already published -- the normal case, the scheduler runs a unit ahead --
@@ -851,8 +865,9 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 if (u.kind == kUnitReduce) continue;
                 const CUtensorMap* tm = &P.tm_a[u.layer];
                 const int a_row = P.m_off + u.m_blk * tile_m + (pair ? static_cast<int>(rank) * a_rows : 0);
-                const bool wait = P.wait_flags && u.layer > P.layer_begin && !u.acquired;
-                if (P.wait_flags && u.layer > P.layer_begin) fence_proxy_async();
+                const bool consumer = P.wait_flags && (u.layer > P.layer_begin || P.wait_first);
+                const bool wait = consumer && !u.acquired;
+                if (consumer) fence_proxy_async();
                 const LayerParams& Lp = P.layer[u.layer > 0 ? u.layer - 1 : 0];
                 const uint32_t target = static_cast<uint32_t>((epoch + 1ull) * static_cast<unsigned long long>(Lp.ready_inc));
                 const uint32_t* ready = wait ? Lp.ready + u.m_blk * Lp.n_blks * nb_mul : nullptr;
@@ -898,7 +913,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                                         if ((n & 255u) == 0) {
                                             if (ld_relaxed_gpu(P.status) != 0) { aborted = true; break; }
                                             if (globaltimer_ns() - t0 > P.timeout_ns) {
-                                                if (lane == 0) atomicCAS(P.status, 0u, kStatusFlagTimeout);
+                                                if (lane == 0) flag_timeout(P.status, P.status_host);
                                                 aborted = true;
                                                 break;
                                             }
@@ -1030,7 +1045,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 if (!u.acquired) {
                     if (r == 0)
                         poll_counter(L.arrive + ctile, static_cast<uint32_t>((epoch + 1ull) * static_cast<unsigned long long>(L.split)),
-                                     P.status, P.timeout_ns, wait_part);
+                                     P.status, P.status_host, P.timeout_ns, wait_part);
                     bar_sync(1, kEpiThreads);  // thread 0's acquire happens-before everybody's loads below
                 }
                 if (r == 0) mbar_arrive(bar_wtaken + 8 * slot);  // late binding: now the scheduler may draw the next ticket
@@ -1109,8 +1124,10 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                     __nanosleep((hsh & 1023u) * 16u);
                 }
                 bar_sync(1, kEpiThreads);
-                if (r == 0) red_release_gpu_add(L.ready + ctile, 1u);  // release: orders the tile before the counter
-                if (r == 0 && P.wait_flags && u.layer + 1 < P.layer_end && P.layer[u.layer + 1].use_queue) {
+                // (test hook MLP_FLAG_DEBUG_DROP_PUBLISH: one producer tile is never published -> its consumers starve -> watchdog)
+                const bool drop = (P.flags & kFlagDebugDropPublish) && u.layer == P.layer_begin && ctile == 0;
+                if (r == 0 && !drop) red_release_gpu_add(L.ready + ctile, 1u);  // release: orders the tile before the counter
+                if (r == 0 && !drop && P.wait_flags && u.layer + 1 < P.layer_end && P.layer[u.layer + 1].use_queue) {
                     // Producer epilogue of the paper's protocol (PAPER.md:95 steps (2)-(4)): look the tile up in the
                     // dependency array, update the scoreboard entry of every group that depends on it, and push the
                     // units of a group whose last dependency this was into the consumer's work queue.

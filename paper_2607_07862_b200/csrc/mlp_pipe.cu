@@ -49,6 +49,14 @@ struct mlp_pipe {
     size_t smem_bytes = 0;
     int pair = 0;      // MLP_FLAG_PAIR: CTA pairs; a WORKER (who draws tickets) is then a pair
     int workers = 0;   // grid, or grid / 2
+    // MLP_FLAG_TWO_KERNEL: every layer is a launch of its own with its own grid (producer / consumer partition of the SMs);
+    // otherwise lgrid[l] = grid and lworkers[l] = workers for every layer
+    int lgrid[kMaxLayers] = {0};
+    int lworkers[kMaxLayers] = {0};
+    bool two_kernel = false;
+    std::vector<cudaStream_t> tk_stream;   // one stream per layer
+    std::vector<cudaEvent_t> tk_done;      // one event per layer
+    PFN_cuStreamWaitValue32_v11070 wait_value32 = nullptr;
     int split[kMaxLayers] = {0};
     int reduce_mode[kMaxLayers] = {0};
     int ready_inc[kMaxLayers] = {0};
@@ -80,6 +88,8 @@ struct mlp_pipe {
     uint32_t* ready[kMaxLayers] = {nullptr};
     unsigned long long* epoch = nullptr;  // [kMaxLayers]
     uint32_t* status = nullptr;
+    uint32_t* status_host = nullptr;      // pinned + mapped mirror of `status`, written by the kernel on a watchdog expiry only
+    uint32_t* status_host_dev = nullptr;  // its device address
     CtaStats* stats = nullptr;  // [kMaxLayers][grid]
     // staging for run_host
     void* stage_X = nullptr;
@@ -94,8 +104,11 @@ struct mlp_pipe {
     // MICROBATCH plumbing
     std::vector<cudaStream_t> side;
     cudaEvent_t ev_fork = nullptr;
+    cudaEvent_t ev_t0 = nullptr, ev_t1 = nullptr;  // autotune of MICROBATCH: fork .. join time
     std::vector<cudaEvent_t> ev_done;  // [L][chunks]
     bool poisoned_state = false;       // a watchdog expiry was seen: counters must be reset
+    unsigned long long tk_epoch = 0;   // MLP_FLAG_TWO_KERNEL: runs since the last reset (= the device epoch when this run starts)
+    bool drop_fired = false;           // MLP_FLAG_DEBUG_DROP_PUBLISH is one-shot: only the handle's first run drops its publish
     unsigned long long runs = 0;
     std::string last_error;
 };
@@ -149,6 +162,18 @@ int encode_2d(mlp_pipe* h, CUtensorMap* out, const void* ptr, int rows, int cols
     return MLP_OK;
 }
 
+// Developer hooks (MLP_PIPE_BOUNDS_<l>, MLP_PIPE_NO_RASTER, MLP_PIPE_DEBUG) exist only in a library built with
+// -DMLP_PIPE_DEBUG_HOOKS (`MLP_PIPE_DEBUG_HOOKS=1 python -m paper_2607_07862_b200.build --force`): the product build never
+// reads its launch plan from the environment.
+const char* debug_env(const char* name) {
+#ifdef MLP_PIPE_DEBUG_HOOKS
+    return getenv(name);
+#else
+    (void)name;
+    return nullptr;
+#endif
+}
+
 int round_up(int a, int b) { return (a + b - 1) / b * b; }
 int ceil_div(int a, int b) { return (a + b - 1) / b; }
 
@@ -159,6 +184,9 @@ int validate_mode(const mlp_mode& m, int M) {
     if (m.tile_m < 0 || m.tile_m % 16 != 0) return MLP_ERR_INVALID;
     if ((m.flags & MLP_FLAG_PAIR) && ((m.flags & MLP_FLAG_WORKQUEUE) || m.tile_n == 2 * kTileN || (m.tile_m % 32) != 0 || (m.grid & 1)))
         return MLP_ERR_UNSUPPORTED;
+    if ((m.flags & MLP_FLAG_TWO_KERNEL) && (m.kind != MLP_CTA_PIPELINED || (m.flags & (MLP_FLAG_WORKQUEUE | MLP_FLAG_PAIR | MLP_FLAG_AUTOTUNE))))
+        return MLP_ERR_UNSUPPORTED;
+    if ((m.flags & MLP_FLAG_MB_CORESIDENT) && m.kind != MLP_MICROBATCH) return MLP_ERR_INVALID;
     if (m.stages < 0 || m.split_k < 0 || m.grid < 0 || m.timeout_ms < 0 || m.w_group < 0 || m.a_stages < 0) return MLP_ERR_INVALID;
     for (int l = 0; l < kMaxLayers; ++l)
         if (m.split_k_layer[l] < 0) return MLP_ERR_INVALID;
@@ -224,7 +252,7 @@ struct Planner {
     }
     // a producer with large tiles whose tiles already fill most of the machine: never split in the modelled search
     bool big_producer(int l) const {
-        return producer_in_launch(l) && reduce_mode_for(2) == kReduceUnits && h->tiles[l] * 10 >= h->workers * 7;
+        return producer_in_launch(l) && reduce_mode_for(2) == kReduceUnits && h->tiles[l] * 10 >= h->lworkers[l] * 7;
     }
     int reduce_mode_for(int sp) const {
         if (sp <= 1) return kReduceNone;
@@ -236,7 +264,7 @@ struct Planner {
     }
     // token columns per reduce unit: about one reduce unit per CTA and layer, at least 16 columns
     int reduce_cols(int l) const {
-        const int chunks = std::max(1, std::min(h->tile_m / 16, (h->workers + h->tiles[l] - 1) / h->tiles[l]));
+        const int chunks = std::max(1, std::min(h->tile_m / 16, (h->lworkers[l] + h->tiles[l] - 1) / h->tiles[l]));
         return ((h->tile_m + chunks - 1) / chunks + 15) / 16 * 16;
     }
 
@@ -276,7 +304,7 @@ struct Planner {
         {
             const int nb = tiles / h->m_blks;
             int i = 0;
-            if (h->m_blks >= 4 && !getenv("MLP_PIPE_NO_RASTER"))
+            if (h->m_blks >= 4 && !debug_env("MLP_PIPE_NO_RASTER"))
                 for (int mg = 0; mg < h->m_blks; mg += kRasterM)
                     for (int n = 0; n < nb; ++n)
                         for (int mb = mg; mb < std::min(h->m_blks, mg + kRasterM); ++mb) order[i++] = mb * nb + n;
@@ -311,7 +339,7 @@ struct Planner {
         }
         // tile-major: interleave.  Tile t's last slice has ticket (t + 1) sp - 1; its reduce units go after
         // ticket (t + 1) sp - 1 + delay of the MMA sequence.
-        const int delay = h->workers + h->workers / 4;
+        const int delay = h->lworkers[l] + h->lworkers[l] / 4;
         std::vector<UnitDesc> merged;
         merged.reserve(out.size() + static_cast<size_t>(tiles) * chunks);
         int next_red = 0;
@@ -336,7 +364,7 @@ struct Planner {
     // and the workers that are streaming weights at the same moment SHARE the HBM bandwidth (a worker alone is
     // limited by its own ring / L2 port / tensor core instead).  Returns the time the last output is stored.
     double makespan(int lb, int le, double cutoff = 1e30) const {
-        const int G = h->workers, R = h->pair ? 2 : h->n_sub, tm = h->tile_m;
+        const int G = h->lworkers[lb], R = h->pair ? 2 : h->n_sub, tm = h->tile_m;
         const double w_bytes = R * static_cast<double>(kWTileBytes), a_bytes = tm * 128.0;
         // per K-block and worker: floor set by the worker's own limits ...
         const double t_cap = std::max({kDramLatencyUs / h->stages, (w_bytes + a_bytes) / kSmBytesPerUs,
@@ -512,7 +540,7 @@ std::string plan_key(const mlp_pipe* h) {
     for (int l = 0; l < h->L; ++l) {
         char name[32];
         snprintf(name, sizeof name, "MLP_PIPE_BOUNDS_%d", l);
-        const char* e = getenv(name);
+        const char* e = debug_env(name);
         k.append(e ? e : "-");
         k.push_back(';');
     }
@@ -522,8 +550,8 @@ std::string plan_key(const mlp_pipe* h) {
 Planner make_planner(mlp_pipe* h) {
     Planner pl;
     pl.h = h;
-    pl.pipelined = h->mode.kind == MLP_CTA_PIPELINED;
-    pl.force_tile_major = (h->mode.flags & (MLP_FLAG_TILE_MAJOR | MLP_FLAG_DEBUG_REVERSE)) != 0;
+    pl.pipelined = h->mode.kind == MLP_CTA_PIPELINED && !h->two_kernel;
+    pl.force_tile_major = (h->mode.flags & (MLP_FLAG_TILE_MAJOR | MLP_FLAG_DEBUG_REVERSE)) != 0 || h->two_kernel;
     for (int l = 0; l < h->L; ++l) pl.kb_total[l] = ceil_div(h->widths[l], kTileK);
     return pl;
 }
@@ -541,7 +569,7 @@ std::vector<std::vector<int>> slice_candidates(const Planner& pl, int l, bool la
     //  * the last layer of a decode-sized problem gets ~12 slices tapering 6:1 (short ragged tail, two gather trips).
     const bool big_producer = !thin && pl.big_producer(l);
     const bool decode_last = !thin && last && !pl.force_tile_major && !pl.producer_in_launch(l) && h->tile_m <= 32 && s_max >= 12 &&
-                             h->tiles[l] * 3 <= h->workers;
+                             h->tiles[l] * 3 <= h->lworkers[l];
     if (big_producer) {
         cand.push_back(pl.uniform(l, 1));
         return cand;
@@ -614,17 +642,31 @@ void resolve(mlp_pipe* h) {
     h->a_stages = ast;
     h->smem_bytes = static_cast<size_t>(st) * w_tile + static_cast<size_t>(ast) * a_tile + kStageBytes + kCtrlBytes + 1024;
     h->grid = m.grid > 0 ? std::min(m.grid, h->num_sms) : h->num_sms;
+    // MICROBATCH, co-resident form (MLP_FLAG_MB_CORESIDENT): layer l of chunk i+1 can only overlap layer l+1 of chunk i
+    // if the launches on the different streams fit on the device TOGETHER -- each gets an equal share of the SMs
+    if (m.kind == MLP_MICROBATCH && (m.flags & MLP_FLAG_MB_CORESIDENT) && m.grid <= 0)
+        h->grid = std::max(1, h->num_sms / std::max(1, std::min(h->L, m.chunks)));
     if (h->pair) h->grid &= ~1;
     h->workers = h->pair ? h->grid / 2 : h->grid;
+    h->two_kernel = m.kind == MLP_CTA_PIPELINED && (m.flags & MLP_FLAG_TWO_KERNEL) && h->L == 2;
+    for (int l = 0; l < kMaxLayers; ++l) {
+        h->lgrid[l] = h->grid;
+        h->lworkers[l] = h->workers;
+    }
+    if (h->two_kernel) {   // producer kernel on s x grid CTAs, consumer kernel on the rest (sm_split; 0 or 1 is read as 1/2)
+        const float sp2 = (m.sm_split <= 0.0f || m.sm_split >= 1.0f) ? 0.5f : m.sm_split;
+        h->lgrid[0] = h->lworkers[0] = std::min(h->grid - 1, std::max(1, static_cast<int>(h->grid * sp2 + 0.5f)));
+        h->lgrid[1] = h->lworkers[1] = h->grid - h->lgrid[0];
+    }
     const float s = (m.sm_split <= 0.0f) ? 1.0f : m.sm_split;
     h->producer_ctas = h->workers;  // (counted in workers)
-    if (m.kind == MLP_CTA_PIPELINED && h->L > 1 && s < 1.0f)
+    if (m.kind == MLP_CTA_PIPELINED && h->L > 1 && s < 1.0f && !h->two_kernel)
         h->producer_ctas = std::min(h->workers, std::max(1, static_cast<int>(h->workers * s + 0.5f)));
 
     Planner pl;
     pl.h = h;
-    pl.pipelined = m.kind == MLP_CTA_PIPELINED;
-    pl.force_tile_major = (m.flags & (MLP_FLAG_TILE_MAJOR | MLP_FLAG_DEBUG_REVERSE)) != 0;
+    pl.pipelined = m.kind == MLP_CTA_PIPELINED && !h->two_kernel;
+    pl.force_tile_major = (m.flags & (MLP_FLAG_TILE_MAJOR | MLP_FLAG_DEBUG_REVERSE)) != 0 || h->two_kernel;
     for (int l = 0; l < h->L; ++l) {
         pl.kb_total[l] = ceil_div(h->widths[l], kTileK);
         h->tiles[l] = ceil_div(h->widths[l + 1], kTileN * (h->pair ? 2 : h->n_sub)) * h->m_blks;
@@ -641,7 +683,7 @@ void resolve(mlp_pipe* h) {
         fixed[l] = sp > 0;
         h->fixed_split[l] = fixed[l];
         if (sp <= 0) {
-            sp = std::min(ceil_div(3 * h->workers, h->tiles[l]), std::max(1, pl.kb_total[l] / kb_min));
+            sp = std::min(ceil_div(3 * h->lworkers[l], h->tiles[l]), std::max(1, pl.kb_total[l] / kb_min));
             if (pl.producer_in_launch(l) && pl.reduce_mode_for(sp) == kReduceLastArriver) sp = std::min(sp, 4);
             if (pl.big_producer(l)) sp = 1;
         }
@@ -686,7 +728,7 @@ void resolve(mlp_pipe* h) {
     for (int l = 0; l < h->L; ++l) {  // experiments: MLP_PIPE_BOUNDS_<l>="0,24,..,<kb_total>" overrides the slices of layer l
         char name[32];
         snprintf(name, sizeof name, "MLP_PIPE_BOUNDS_%d", l);
-        const char* e = getenv(name);
+        const char* e = debug_env(name);
         if (!e) continue;
         std::vector<int> b;
         for (const char* q = e; *q;) {
@@ -711,7 +753,7 @@ void resolve(mlp_pipe* h) {
     if (pl.pipelined) h->model_us = pl.makespan(0, h->L);
     else
         for (int l = 0; l < h->L; ++l) h->model_us += pl.makespan(l, l + 1) * (m.kind == MLP_MICROBATCH ? m.chunks : 1);
-    if (getenv("MLP_PIPE_DEBUG")) {
+    if (debug_env("MLP_PIPE_DEBUG")) {
         fprintf(stderr, "[mlp_pipe] M=%d tile %dx%d stages %d/%d acc %d grid %d mode %d: model %.1f us\n", h->M, kTileN * h->n_sub,
                 h->tile_m, h->stages, h->a_stages, h->acc_stages, h->grid, m.kind, pl.pipelined ? pl.makespan(0, h->L) : -1.0);
         for (int l = 0; l < h->L; ++l) {
@@ -738,7 +780,7 @@ int build_base_params(mlp_pipe* h) {
         Lp.publish = l < h->L - 1 ? 1 : 0;
         Lp.reduce_mode = h->reduce_mode[l];
         {   // do the first `grid` tickets follow the closed form (tile-major, equal slices)?
-            const int sp = h->split[l], n = std::min<int>(h->workers, static_cast<int>(h->table[l].size()));
+            const int sp = h->split[l], n = std::min<int>(h->lworkers[l], static_cast<int>(h->table[l].size()));
             bool ok = sp <= 255;
             for (int t = 0; t < n && ok; ++t) {
                 const UnitDesc& d = h->table[l][t];
@@ -790,6 +832,7 @@ int build_base_params(mlp_pipe* h) {
     P.w_group = std::max(1, std::min(h->mode.w_group > 0 ? h->mode.w_group : 1, h->stages));
     P.flags = h->mode.flags;
     P.status = h->status;
+    P.status_host = h->status_host_dev;
     P.timeout_ns = static_cast<unsigned long long>(h->mode.timeout_ms > 0 ? h->mode.timeout_ms : 2000) * 1000000ull;
     return MLP_OK;
 }
@@ -799,7 +842,9 @@ int reset_state(mlp_pipe* h, cudaStream_t s) {
     for (int l = 0; l < kMaxLayers; ++l)
         if (h->q_state[l]) CUDA_TRY(h, cudaMemsetAsync(h->q_state[l], 0, h->q_state_words[l] * sizeof(uint32_t), s));
     CUDA_TRY(h, cudaMemsetAsync(h->epoch, 0, kMaxLayers * sizeof(unsigned long long), s));
+    h->tk_epoch = 0;
     CUDA_TRY(h, cudaMemsetAsync(h->status, 0, sizeof(uint32_t), s));
+    if (h->status_host) *reinterpret_cast<volatile uint32_t*>(h->status_host) = 0u;  // (callers have synchronised the device)
     CUDA_TRY(h, cudaMemsetAsync(h->stats, 0, sizeof(CtaStats) * kMaxLayers * h->grid, s));
     return MLP_OK;
 }
@@ -826,7 +871,7 @@ int lookup_tmap(mlp_pipe* h, TmapCacheEntry* cache, int* next, const void* ptr, 
 // Ticket bookkeeping of one launch over layers [layer_begin, layer_end) (see kernel.cuh, scheduler):
 // CTAs that START on a layer take unit `rank` statically, everyone else draws atomically.
 void set_ticket_params(const mlp_pipe* h, KernelParams& P) {
-    const int b = P.layer_begin, e = P.layer_end, G = h->workers, p = P.producer_ctas;
+    const int b = P.layer_begin, e = P.layer_end, G = h->lworkers[P.layer_begin], p = P.producer_ctas;
     for (int l = b; l < e; ++l) {
         const int statics = l == b ? p : (l == b + 1 ? G - p : 0);
         const int arrivals = l == b ? 0 : (l == b + 1 ? p : G);
@@ -838,13 +883,27 @@ void set_ticket_params(const mlp_pipe* h, KernelParams& P) {
 int launch(mlp_pipe* h, KernelParams& P, cudaStream_t s) {
     set_ticket_params(h, P);
     cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3(h->grid);
+    cfg.gridDim = dim3(h->lgrid[P.layer_begin]);
     cfg.blockDim = dim3(kThreads);
     cfg.dynamicSmemBytes = h->smem_bytes;
     cfg.stream = s;
-    cudaLaunchAttribute attr[2];
+    cudaLaunchAttribute attr[3];
     cfg.attrs = nullptr;
     cfg.numAttrs = 0;
+    // Co-residency.  A CTA that waits (consumer prologue, reduce unit) waits on units that OTHER CTAs of this launch own --
+    // the first unit of every CTA is static -- so every CTA of the grid must be resident, which grid <= #SMs guarantees only
+    // on an otherwise idle GPU.  A cooperative launch makes it a guarantee: the grid starts only when all of it fits at once
+    // (behind another kernel, or a second handle on another stream, it queues instead of deadlocking until the watchdog).
+    bool waits = P.wait_flags != 0;
+    for (int l = P.layer_begin; l < P.layer_end; ++l) waits = waits || P.layer[l].reduce_mode == kReduceUnits;
+    // (not for launches that are MEANT to share the device with a sibling launch of the same handle: the two-kernel
+    // pipeline and co-resident micro-batches size their grids so that the siblings fit together)
+    if (waits && !(h->mode.flags & (MLP_FLAG_NO_COOPERATIVE | MLP_FLAG_PDL | MLP_FLAG_TWO_KERNEL | MLP_FLAG_MB_CORESIDENT))) {
+        attr[cfg.numAttrs].id = cudaLaunchAttributeCooperative;
+        attr[cfg.numAttrs].val.cooperative = 1;
+        cfg.attrs = attr;
+        ++cfg.numAttrs;
+    }
     if (h->pair) {  // CTA pairs: clusters of 2 (same TPC), required by tcgen05 cta_group::2
         attr[cfg.numAttrs].id = cudaLaunchAttributeClusterDimension;
         attr[cfg.numAttrs].val.clusterDim.x = 2;
@@ -975,6 +1034,14 @@ int create_impl(mlp_pipe** out, int M, int L, const int* widths, int dtype, int 
     h->dev = dev;
     h->num_sms = prop.multiProcessorCount;
     resolve(h);
+    for (int l = 0; l < L; ++l) {  // the unit table stores tile ids and K-block bounds in 16 bits, the K-slice index in 8
+        const long long tiles128 = static_cast<long long>(ceil_div(widths[l + 1], kTileN)) * h->m_blks;
+        if (tiles128 > 65535 || ceil_div(widths[l], kTileK) > 65535) {
+            delete h;
+            return fail(nullptr, MLP_ERR_UNSUPPORTED, "layer %d: %lld output tiles / %d K-blocks exceed the unit table's 16-bit fields", l,
+                        tiles128, ceil_div(widths[l], kTileK));
+        }
+    }
     if (h->pair && ((h->tile_m % 32) != 0 || h->grid < 2)) {
         const int tm = h->tile_m;
         delete h;
@@ -1016,16 +1083,41 @@ int create_impl(mlp_pipe** out, int M, int L, const int* widths, int dtype, int 
     }
     CREATE_TRY(cudaMalloc(&h->epoch, kMaxLayers * sizeof(unsigned long long)));
     CREATE_TRY(cudaMalloc(&h->status, sizeof(uint32_t)));
+    CREATE_TRY(cudaHostAlloc(reinterpret_cast<void**>(&h->status_host), sizeof(uint32_t), cudaHostAllocMapped));
+    *h->status_host = 0u;
+    CREATE_TRY(cudaHostGetDevicePointer(reinterpret_cast<void**>(&h->status_host_dev), h->status_host, 0));
     CREATE_TRY(cudaMalloc(&h->stats, sizeof(CtaStats) * kMaxLayers * h->grid));
+    if ((m.flags & MLP_FLAG_TWO_KERNEL) && !h->two_kernel) {
+        mlp_pipe_destroy(h);
+        return fail(nullptr, MLP_ERR_UNSUPPORTED, "MLP_FLAG_TWO_KERNEL needs a 2-layer handle");
+    }
+    if (h->two_kernel) {
+        void* fp = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuStreamWaitValue32", &fp, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess || !fp) {
+            mlp_pipe_destroy(h);
+            return fail(nullptr, MLP_ERR_UNSUPPORTED, "cuStreamWaitValue32 entry point not found");
+        }
+        h->wait_value32 = reinterpret_cast<PFN_cuStreamWaitValue32_v11070>(fp);
+        h->tk_stream.resize(L, nullptr);
+        h->tk_done.resize(L, nullptr);
+        for (int l = 0; l < L; ++l) {
+            CREATE_TRY(cudaStreamCreateWithFlags(&h->tk_stream[l], cudaStreamNonBlocking));
+            CREATE_TRY(cudaEventCreateWithFlags(&h->tk_done[l], cudaEventDisableTiming));
+        }
+        CREATE_TRY(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
+    }
     if (m.kind == MLP_MICROBATCH) {
         h->side.resize(L, nullptr);
         for (int l = 0; l < L; ++l) CREATE_TRY(cudaStreamCreateWithFlags(&h->side[l], cudaStreamNonBlocking));
         CREATE_TRY(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
+        CREATE_TRY(cudaEventCreate(&h->ev_t0));
+        CREATE_TRY(cudaEventCreate(&h->ev_t1));
         h->ev_done.resize(static_cast<size_t>(L) * m.chunks, nullptr);
         for (auto& e : h->ev_done) CREATE_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     }
     rc = install_plan(h);
-    h->tuned = !(m.flags & MLP_FLAG_AUTOTUNE) || m.kind == MLP_MICROBATCH;
+    h->tuned = !(m.flags & MLP_FLAG_AUTOTUNE);
     if (rc) {
         g_create_error = h->last_error;
         mlp_pipe_destroy(h);
@@ -1049,13 +1141,22 @@ int run_core(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStre
     if (!W) return fail(h, MLP_ERR_INVALID, "W is NULL");
     for (int l = 0; l < h->L; ++l)
         if ((rc = check_ptr(h, W[l], "W[l]"))) return rc;
+    // A watchdog expiry of an earlier run shows up here without a device round trip: the kernel mirrors its status word into
+    // pinned host memory.  Runs already queued behind the expired one terminate (every wait gives up at once while the
+    // status is set) with undefined output; the first call after the expiry reports it and resets the handle.
+    if (h->status_host && *reinterpret_cast<volatile uint32_t*>(h->status_host) != 0u) h->poisoned_state = true;
     if (h->poisoned_state) {
         CUDA_TRY(h, cudaDeviceSynchronize());
         if ((rc = reset_state(h, s))) return rc;
+        CUDA_TRY(h, cudaStreamSynchronize(s));
         h->poisoned_state = false;
         return fail(h, MLP_ERR_TIMEOUT, "a previous run hit the flag watchdog; the handle has been reset");
     }
     KernelParams P = h->base;
+    if (P.flags & MLP_FLAG_DEBUG_DROP_PUBLISH) {  // test hook, one-shot: run 1 starves, the runs after the reset are clean
+        if (h->drop_fired) P.flags &= ~static_cast<uint32_t>(MLP_FLAG_DEBUG_DROP_PUBLISH);
+        h->drop_fired = true;
+    }
     if ((rc = lookup_tmap(h, h->cache_x, &h->cache_x_next, X, h->M, h->widths[0], h->pair ? h->tile_m / 2 : h->tile_m, &P.tm_a[0]))) return rc;
     for (int l = 0; l < h->L; ++l)
         if ((rc = lookup_tmap(h, h->cache_w[l], &h->cache_w_next[l], W[l], h->widths[l + 1], h->widths[l], kTileN * h->n_sub, &P.tm_w[l])))
@@ -1063,7 +1164,40 @@ int run_core(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStre
     P.layer[h->L - 1].out = static_cast<__nv_bfloat16*>(Y);
 
     const int kind = h->mode.kind;
-    if (kind == MLP_CTA_PIPELINED) {
+    if (h->two_kernel) {
+        // The paper's host organisation on ONE GPU ("producer and consumer kernels are launched onto separate
+        // streams"): the producer layer is a kernel on stream A over s x grid SMs, the consumer layer a kernel on
+        // stream B over the rest, and B is gated by cuStreamWaitValue32 on the FIRST ready counter reaching this run's
+        // target -- the consumer kernel does not occupy its SMs before there is anything to consume.  Same kernel, same
+        // counters; the consumer's first layer polls (wait_first) exactly as a consumer unit inside one launch does.
+        cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(s, &cap) == cudaSuccess && cap != cudaStreamCaptureStatusNone)
+            return fail(h, MLP_ERR_UNSUPPORTED, "MLP_FLAG_TWO_KERNEL cannot be captured (the wait value is computed per run on the host)");
+        CUDA_TRY(h, cudaEventRecord(h->ev_fork, s));
+        for (int l = 0; l < 2; ++l) {
+            CUDA_TRY(h, cudaStreamWaitEvent(h->tk_stream[l], h->ev_fork, 0));
+            P.layer_begin = l;
+            P.layer_end = l + 1;
+            P.m_off = 0;
+            P.m_end = h->M;
+            P.wait_flags = 1;
+            P.wait_first = l > 0 ? 1 : 0;
+            P.producer_ctas = h->lworkers[l];
+            P.epoch_counter = h->epoch + l;
+            P.stats = h->stats + static_cast<size_t>(l) * h->grid;
+            if (l > 0) {
+                const uint32_t target = static_cast<uint32_t>((h->tk_epoch + 1ull) * static_cast<unsigned long long>(h->ready_inc[0]));
+                const uint32_t* first = h->ready[0] + h->table[0][0].tile;   // the tile of ticket 0 turns first
+                const CUresult r = h->wait_value32(reinterpret_cast<CUstream>(h->tk_stream[l]), reinterpret_cast<CUdeviceptr>(first), target,
+                                                   CU_STREAM_WAIT_VALUE_GEQ);
+                if (r != CUDA_SUCCESS) return fail(h, MLP_ERR_CUDA, "cuStreamWaitValue32 failed (%d)", static_cast<int>(r));
+            }
+            if ((rc = launch(h, P, h->tk_stream[l]))) return rc;
+            CUDA_TRY(h, cudaEventRecord(h->tk_done[l], h->tk_stream[l]));
+        }
+        for (int l = 0; l < 2; ++l) CUDA_TRY(h, cudaStreamWaitEvent(s, h->tk_done[l], 0));
+        h->tk_epoch++;
+    } else if (kind == MLP_CTA_PIPELINED) {
         // one persistent launch; tickets order all units of layer l before those of layer l+1
         P.layer_begin = 0;
         P.layer_end = h->L;
@@ -1115,15 +1249,18 @@ int run_core(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStre
     return MLP_OK;
 }
 
+// Launch classes of a run: 1 (one persistent launch over all layers) or one per layer.
+int launch_classes(const mlp_pipe* h) { return h->mode.kind == MLP_CTA_PIPELINED && !h->two_kernel ? 1 : h->L; }
+
 // In-kernel span of the most recent run: per launch class, last CTA exit - first CTA start (globaltimer), summed.
 int last_span_us(mlp_pipe* h, double* out) {
-    const int classes = h->mode.kind == MLP_CTA_PIPELINED ? 1 : h->L;
+    const int classes = launch_classes(h);
     std::vector<CtaStats> cs(static_cast<size_t>(classes) * h->grid);
     CUDA_TRY(h, cudaMemcpy(cs.data(), h->stats, cs.size() * sizeof(CtaStats), cudaMemcpyDeviceToHost));
     double total = 0.0;
     for (int c = 0; c < classes; ++c) {
         unsigned long long t0 = ~0ull, t1 = 0;
-        for (int b = 0; b < h->grid; ++b) {
+        for (int b = 0; b < h->lgrid[classes == 1 ? 0 : c]; ++b) {
             const CtaStats& st = cs[static_cast<size_t>(c) * h->grid + b];
             t0 = std::min(t0, st.ts[0]);
             t1 = std::max(t1, st.ts[7]);
@@ -1167,11 +1304,20 @@ int autotune(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStre
         int r = install_plan(h);
         if (r) return r;
         double best = 1e30;
-        for (int i = 0; i < 4; ++i) {  // first run warms the tensor maps / instruction cache
+        const bool by_events = h->mode.kind == MLP_MICROBATCH;  // launches on several streams overlap: time the fork .. join
+        for (int i = 0; i < (by_events ? 6 : 4); ++i) {  // first run warms the tensor maps / instruction cache
+            if (by_events) CUDA_TRY(h, cudaEventRecord(h->ev_t0, s));
             if ((r = run_core(h, X, W, Y, s))) return r;
+            if (by_events) CUDA_TRY(h, cudaEventRecord(h->ev_t1, s));
             CUDA_TRY(h, cudaStreamSynchronize(s));
             double t;
-            if ((r = last_span_us(h, &t))) return r;
+            if (by_events) {
+                float ms = 0.0f;
+                CUDA_TRY(h, cudaEventElapsedTime(&ms, h->ev_t0, h->ev_t1));
+                t = ms * 1e3;
+            } else if ((r = last_span_us(h, &t))) {
+                return r;
+            }
             if (i > 0) best = std::min(best, t);
         }
         *us = best;
@@ -1196,7 +1342,7 @@ int autotune(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStre
                     pl.build_table(l, c, h->table[l], h->reduce_mode[l], h->ready_inc[l]);
                     double t;
                     if ((r = measure(&t))) return r;
-                    if (t < best_us - 0.05 * n_launch) {
+                    if (t < best_us - (h->mode.kind == MLP_MICROBATCH ? 1.0 : 0.05 * n_launch)) {
                         best_us = t;
                         best = c;
                         improved = true;
@@ -1245,7 +1391,7 @@ int autotune(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStre
         v[h->L] = {best_tile_n};
         g_plan_cache[key + "#tuned"] = v;
     }
-    if (getenv("MLP_PIPE_DEBUG")) {
+    if (debug_env("MLP_PIPE_DEBUG")) {
         fprintf(stderr, "[mlp_pipe] autotuned: %.1f us in-kernel span; tile_n %d;", best_us, best_tile_n);
         for (int l = 0; l < h->L; ++l) {
             fprintf(stderr, " L%d:", l);
@@ -1382,7 +1528,7 @@ int mlp_pipe_stats(mlp_pipe* h, mlp_stats* out, size_t bytes) {
     st.stages = h->stages;
     st.tile_m = h->tile_m;
     st.tile_n = kTileN * (h->pair ? 2 : h->n_sub);
-    st.producer_ctas = h->producer_ctas;
+    st.producer_ctas = h->two_kernel ? h->lgrid[0] : h->producer_ctas;
     for (int l = 0; l < h->L; ++l) {
         st.split_k[l] = h->split[l];
         st.units[l] = static_cast<int>(h->table[l].size());
@@ -1391,12 +1537,12 @@ int mlp_pipe_stats(mlp_pipe* h, mlp_stats* out, size_t bytes) {
     CUDA_TRY(h, cudaMemcpy(&st.status, h->status, sizeof(uint32_t), cudaMemcpyDeviceToHost));
     unsigned long long ep[kMaxLayers];
     CUDA_TRY(h, cudaMemcpy(ep, h->epoch, sizeof ep, cudaMemcpyDeviceToHost));
-    st.runs = ep[0] / h->grid;
-    const int classes = h->mode.kind == MLP_CTA_PIPELINED ? 1 : h->L;
+    st.runs = ep[0] / h->lgrid[0];
+    const int classes = launch_classes(h);
     std::vector<CtaStats> cs(static_cast<size_t>(classes) * h->grid);
     CUDA_TRY(h, cudaMemcpy(cs.data(), h->stats, cs.size() * sizeof(CtaStats), cudaMemcpyDeviceToHost));
     for (int c = 0; c < classes; ++c)
-        for (int b = 0; b < h->grid; ++b) {
+        for (int b = 0; b < h->lgrid[classes == 1 ? 0 : c]; ++b) {
             const CtaStats& s = cs[static_cast<size_t>(c) * h->grid + b];
             st.flag_stall_cycles_sum += s.stall_cycles;
             st.flag_stall_cycles_max = std::max<uint64_t>(st.flag_stall_cycles_max, s.stall_cycles);
@@ -1412,8 +1558,8 @@ int mlp_pipe_stats(mlp_pipe* h, mlp_stats* out, size_t bytes) {
     CUDA_TRY(h, cudaMemcpy(cw.data(), h->counters, cw.size() * sizeof(uint32_t), cudaMemcpyDeviceToHost));
     bool ok = st.status == 0;
     for (int l = 0; l < h->L && ok; ++l) {
-        const unsigned long long e = (h->mode.kind == MLP_CTA_PIPELINED ? ep[0] : ep[l]) / h->grid;
-        const int arrivals = h->mode.kind != MLP_CTA_PIPELINED || l == 0 ? 0 : (l == 1 ? h->producer_ctas : h->workers);
+        const unsigned long long e = (classes == 1 ? ep[0] : ep[l]) / h->lgrid[classes == 1 ? 0 : l];
+        const int arrivals = classes != 1 || l == 0 ? 0 : (l == 1 ? h->producer_ctas : h->workers);
         const uint32_t* tk = cw.data() + (h->ticket[l] - h->counters);
         const uint32_t* ar = cw.data() + (h->arrive[l] - h->counters);
         const uint32_t* rd = cw.data() + (h->ready[l] - h->counters);
@@ -1451,7 +1597,7 @@ int mlp_pipe_stats(mlp_pipe* h, mlp_stats* out, size_t bytes) {
 int mlp_pipe_cta_records(mlp_pipe* h, int cls, mlp_cta_record* out, int max_records, int* n_out) {
     static_assert(sizeof(mlp_cta_record) == sizeof(CtaStats), "mlp_cta_record must mirror CtaStats");
     if (!h || !out || !n_out || max_records < 0) return MLP_ERR_INVALID;
-    const int classes = h->mode.kind == MLP_CTA_PIPELINED ? 1 : h->L;
+    const int classes = launch_classes(h);
     if (cls < 0 || cls >= classes) return fail(h, MLP_ERR_INVALID, "bad launch class %d", cls);
     CUDA_TRY(h, cudaDeviceSynchronize());
     const int n = std::min(max_records, h->grid);
@@ -1474,15 +1620,28 @@ void mlp_pipe_destroy(mlp_pipe* h) {
     if (h->counters) cudaFree(h->counters);
     if (h->epoch) cudaFree(h->epoch);
     if (h->status) cudaFree(h->status);
+    if (h->status_host) cudaFreeHost(h->status_host);
     if (h->stats) cudaFree(h->stats);
     if (h->stage_X) cudaFree(h->stage_X);
     if (h->stage_Y) cudaFree(h->stage_Y);
     for (auto s : h->side)
         if (s) cudaStreamDestroy(s);
+    for (auto s : h->tk_stream)
+        if (s) cudaStreamDestroy(s);
+    for (auto e : h->tk_done)
+        if (e) cudaEventDestroy(e);
     if (h->ev_fork) cudaEventDestroy(h->ev_fork);
+    if (h->ev_t0) cudaEventDestroy(h->ev_t0);
+    if (h->ev_t1) cudaEventDestroy(h->ev_t1);
     for (auto e : h->ev_done)
         if (e) cudaEventDestroy(e);
     delete h;
+}
+
+static bool fits_unit_table(const mlp_pipe& h) {
+    for (int l = 0; l < h.L; ++l)
+        if (static_cast<long long>(ceil_div(h.widths[l + 1], kTileN)) * h.m_blks > 65535 || ceil_div(h.widths[l], kTileK) > 65535) return false;
+    return true;
 }
 
 int mlp_pipe_plan(int M, int n_layers, const int* widths, const mlp_mode* mode, int num_sms, mlp_plan* out) {
@@ -1500,7 +1659,9 @@ int mlp_pipe_plan(int M, int n_layers, const int* widths, const mlp_mode* mode, 
     for (int l = 0; l <= n_layers; ++l) h.widths[l] = widths[l];
     h.mode = m;
     h.num_sms = num_sms;
+    if (M > 256 * 65535) return MLP_ERR_UNSUPPORTED;
     resolve(&h);
+    if (!fits_unit_table(h)) return MLP_ERR_UNSUPPORTED;
     memset(out, 0, sizeof *out);
     out->tile_m = h.tile_m;
     out->tile_n = kTileN * (h.pair ? 2 : h.n_sub);
@@ -1540,7 +1701,9 @@ int mlp_pipe_plan_units(int M, int n_layers, const int* widths, const mlp_mode* 
     for (int l = 0; l <= n_layers; ++l) h.widths[l] = widths[l];
     h.mode = m;
     h.num_sms = num_sms;
+    if (M > 256 * 65535) return MLP_ERR_UNSUPPORTED;
     resolve(&h);
+    if (!fits_unit_table(h)) return MLP_ERR_UNSUPPORTED;
     const std::vector<UnitDesc>& t = h.table[layer];
     const int n = std::min<int>(max_units, static_cast<int>(t.size()));
     for (int i = 0; i < n; ++i) {

@@ -72,15 +72,6 @@ def test_mma_issue_loop_has_no_per_instruction_elect_loops():
         assert "BRA.U.ANY" not in window, "UTCHMMA inside an elect loop:\n" + "\n".join(lines[i - 2:i + 4])
 
 
-def test_mma_issue_microbenchmark_compiles(tmp_path):
-    """csrc/bench_mma_issue.cu (developer microbenchmark behind profiles/r1d_mma_issue_microbench.txt) still builds for sm_100a."""
-    nvcc = "/usr/local/cuda/bin/nvcc"
-    if not os.path.exists(nvcc):
-        pytest.skip("nvcc not installed")
-    src = os.path.join(ROOT, "paper_2607_07862_b200", "csrc", "bench_mma_issue.cu")
-    subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-c", src, "-o", str(tmp_path / "b.o")], check=True)
-
-
 def test_header_compiles_as_plain_c(tmp_path):
     src = tmp_path / "t.c"
     src.write_text('#include "mlp_pipe.h"\nint main(void){ mlp_mode m = {0}; mlp_stats s; mlp_cta_record r; (void)m; (void)s; (void)r; '

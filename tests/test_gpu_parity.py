@@ -110,26 +110,6 @@ def test_m_gt_256_microbatch_and_split():
 
 
 # ---------------------------------------------------------------- BASELINE.json full sizes
-def sampled_rows_check(ci, mode, rows, x_scale="unit"):
-    """Full-size run in the launch configuration bench.py times; the oracle recomputes a sample of
-    token rows (rows are independent, so each sampled row is the oracle's complete answer for it)."""
-    cfg = inputs.CONFIGS[ci]
-    X, Ws = inputs.make_inputs(cfg, x_scale=x_scale)
-    rows = sorted(set(r % cfg.M for r in rows))
-    outs, _ = oracle.mlp_chain(inputs.as_u16(X)[rows].copy(), [inputs.as_u16(w) for w in Ws], cfg.act)
-    got, hs, st = run_gpu(cfg, mode, X, Ws)
-    assert st.status == 0 and st.ready_ok == 1
-    worst = 0.0
-    for l, h in enumerate(hs):
-        e = oracle.rel_err(h[rows], outs[l])
-        assert e["nan"] == 0 and e["err"] <= TOL, (l, e)
-        worst = max(worst, e["err"])
-    e = oracle.rel_err(got[rows], outs[-1])
-    assert e["nan"] == 0 and e["err"] <= TOL, e
-    assert not np.isnan(oracle.u16_to_f64(got)).any()
-    return max(worst, e["err"]), st
-
-
 def test_cfg1_full_every_element():
     """configs[1] (the bench workload), M = 16: every element against the oracle, all three modes."""
     cfg = inputs.CONFIGS[1]
@@ -138,21 +118,30 @@ def test_cfg1_full_every_element():
     check(cfg, B.make_mode(P), x_scale="fan_in")
 
 
-def test_cfg2_full_sampled_rows():
-    for mode in (B.make_mode(P), B.make_mode(S), B.make_mode(MB, chunks=4), B.make_mode(P, sm_split=0.5)):
-        sampled_rows_check(2, mode, rows=[0, 1, 17, 100, 127, 128, 200, 255])
+FULL_VARIANTS = {
+    # what bench.py times: the measured plan search on the first run, then the tuned plan
+    "pipe_autotuned": lambda: (B.make_mode(P, flags=B.MLP_FLAG_AUTOTUNE), "unit"),
+    "pipe_modelled": lambda: (B.make_mode(P), "unit"),
+    "seq": lambda: (B.make_mode(S), "unit"),
+    "seq_autotuned_pdl": lambda: (B.make_mode(S, flags=B.MLP_FLAG_AUTOTUNE | B.MLP_FLAG_PDL), "unit"),
+    "mb2": lambda: (B.make_mode(MB, chunks=2), "unit"),
+    "mb4": lambda: (B.make_mode(MB, chunks=4), "unit"),
+    "pipe_half": lambda: (B.make_mode(P, sm_split=0.5), "unit"),
+    # reading c4, the literal alternative: X ~ N(0, 1/K)
+    "pipe_autotuned_fan_in": lambda: (B.make_mode(P, flags=B.MLP_FLAG_AUTOTUNE), "fan_in"),
+}
 
 
-def test_cfg3_full_sampled_rows():
-    for mode in (B.make_mode(P), B.make_mode(S)):
-        sampled_rows_check(3, mode, rows=[0, 63, 64, 127])
-
-
-def test_cfg4_chain_full_sampled_rows():
-    """configs[4]: 4 layers, every layer pair linked by ready counters."""
-    for mode in (B.make_mode(P), B.make_mode(S), B.make_mode(P, sm_split=0.5)):
-        err, st = sampled_rows_check(4, mode, rows=[0, 31, 77, 127])
-        assert st.n_layers == 4
+@pytest.mark.parametrize("variant", list(FULL_VARIANTS))
+@pytest.mark.parametrize("ci", [2, 3, 4])
+def test_full_size_every_element(ci, variant):
+    """BASELINE.json configs[2..4] at full size, EVERY element of Y and of every hidden activation H_l against the oracle
+    (the full oracle costs 3-6 s per config and is cached): CTA_PIPELINED with the autotuned plan (the launch configuration
+    bench.py times) and with the modelled plan, SEQUENTIAL (plain and autotuned + PDL), MICROBATCH, a consumer-first
+    split, and the second reading of the X scale (DESIGN.md c4)."""
+    mode, x_scale = FULL_VARIANTS[variant]()
+    st = check(inputs.CONFIGS[ci], mode, x_scale=x_scale)
+    assert st.n_layers == inputs.CONFIGS[ci].n_layers
 
 
 def test_exact_mode_on_llama_shape_with_certificate():
@@ -257,27 +246,151 @@ def test_run_host_matches_device_path():
     p.close()
 
 
-def test_watchdog_turns_a_hang_into_timeout():
-    """A consumer-only launch (no producer ever publishes) must end with MLP_ERR_TIMEOUT, not hang."""
+@pytest.mark.parametrize("extra", [0, B.MLP_FLAG_WORKQUEUE, B.MLP_FLAG_PAIR])
+def test_watchdog_turns_a_hang_into_timeout(extra):
+    """MLP_FLAG_DEBUG_DROP_PUBLISH: the producer of tile 0 never publishes on the handle's FIRST run, so the consumers of
+    that tile starve.  The flag-poll watchdog must end the kernel (no hang), MLP_ERR_TIMEOUT must be reported -- by
+    mlp_pipe_stats, and by the next mlp_pipe_run WITHOUT any stats call (the kernel mirrors its status word into pinned
+    host memory) --, the handle must be reset, and the runs after that must be bit-exact again."""
     cfg = inputs.get_config(0, "exact")
-    X, Ws, _, _ = oracle_outs(cfg)
-    # grid = 1 and sm_split so small that the only CTA is a producer is the normal case; to starve the
-    # consumer we run a 1-CTA grid in reverse order with the reducer waiting on nothing -> instead use the
-    # documented hook: timeout_ms tiny + DEBUG_DELAY makes producers slower than the watchdog.
-    p = B.MlpPipe(cfg.M, cfg.widths, cfg.act, B.make_mode(P, sm_split=0.5, flags=B.MLP_FLAG_DEBUG_DELAY, timeout_ms=1))
-    p.run(X.cuda(), [w.cuda() for w in Ws])
-    torch.cuda.synchronize()          # the kernel must terminate either way
-    try:
-        st = p.stats()
-        assert st.status == 0         # fast enough: no expiry, nothing to check
-    except B.MlpError as e:
-        assert e.status == B.MLP_ERR_TIMEOUT
-        with pytest.raises(B.MlpError):
-            p.run(X.cuda(), [w.cuda() for w in Ws])      # reports the reset once
-        Y = p.run(X.cuda(), [w.cuda() for w in Ws])        # and works again afterwards
-        torch.cuda.synchronize()
-        assert p.stats().status == 0
+    X, Ws, outs, _ = oracle_outs(cfg)
+    Xd, Wd = X.cuda(), [w.cuda() for w in Ws]
+    flags = B.MLP_FLAG_DEBUG_DROP_PUBLISH | extra
+    # (a) reported by stats
+    p = B.MlpPipe(cfg.M, cfg.widths, cfg.act, B.make_mode(P, flags=flags, timeout_ms=20))
+    p.run(Xd, Wd)
+    torch.cuda.synchronize()          # the kernel terminates although one tile is never published
+    with pytest.raises(B.MlpError) as e:
+        p.stats()
+    assert e.value.status == B.MLP_ERR_TIMEOUT
+    with pytest.raises(B.MlpError) as e:
+        p.run(Xd, Wd)                 # reports the reset once
+    assert e.value.status == B.MLP_ERR_TIMEOUT
+    for _ in range(3):
+        p.poison_hidden(0x7FC0)
+        Y = p.run(Xd, Wd)             # the hook is one-shot: clean runs from here on
+        assert np.array_equal(inputs.as_u16(Y.cpu()), outs[-1])
+    st = p.stats()
+    assert st.status == 0 and st.ready_ok == 1 and st.runs == 3
     p.close()
+    # (b) reported on the run path alone
+    p = B.MlpPipe(cfg.M, cfg.widths, cfg.act, B.make_mode(P, flags=flags, timeout_ms=20))
+    p.run(Xd, Wd)
+    torch.cuda.synchronize()
+    with pytest.raises(B.MlpError) as e:
+        p.run(Xd, Wd)
+    assert e.value.status == B.MLP_ERR_TIMEOUT
+    Y = p.run(Xd, Wd)
+    assert np.array_equal(inputs.as_u16(Y.cpu()), outs[-1])
+    assert p.stats().ready_ok == 1
+    p.close()
+
+
+def test_two_pipelined_handles_on_two_streams():
+    """Co-residency (include/mlp_pipe.h): a waiting CTA waits on units owned by other CTAs of its launch, so a launch must
+    never start partially.  Two CTA_PIPELINED handles fed from two streams at the same time: with cooperative launches
+    each grid starts only when all of it fits, nothing starves, nothing times out, every result is bit-exact."""
+    cfg = inputs.Config("two_handles", 64, (1024, 4096, 1024), B.MLP_ACT_RELU, "exact", 5)
+    X, Ws, outs, _ = oracle_outs(cfg)
+    Xd, Wd = X.cuda(), [w.cuda() for w in Ws]
+    ps = [B.MlpPipe(cfg.M, cfg.widths, cfg.act, B.make_mode(P, split_k=4, timeout_ms=500)) for _ in range(2)]
+    streams = [torch.cuda.Stream() for _ in range(2)]
+    Ys = [torch.zeros((cfg.M, cfg.widths[-1]), dtype=torch.bfloat16, device="cuda") for _ in range(2)]
+    torch.cuda.synchronize()
+    for i in range(200):
+        for k in range(2):
+            with torch.cuda.stream(streams[k]):
+                ps[k].run(Xd, Wd, Ys[k], stream=streams[k])
+    torch.cuda.synchronize()
+    for k in range(2):
+        st = ps[k].stats()
+        assert st.status == 0 and st.ready_ok == 1 and st.runs == 200
+        assert np.array_equal(inputs.as_u16(Ys[k].cpu()), outs[-1])
+        ps[k].close()
+
+
+TK = B.MLP_FLAG_TWO_KERNEL
+
+
+@pytest.mark.parametrize("kw", [dict(), dict(sm_split=0.25, split_k=4), dict(sm_split=0.75, split_k=2), dict(split_k_layer=[2, 8]),
+                                dict(flags=B.MLP_FLAG_DEBUG_DELAY, split_k=4), dict(flags=B.MLP_FLAG_DEBUG_DELAY | B.MLP_FLAG_DEBUG_REVERSE),
+                                dict(flags=B.MLP_FLAG_ACQUIRE_LOADS, split_k=4)], ids=[str(i) for i in range(7)])
+def test_two_kernel_stream_wait_pipeline(kw):
+    """MLP_FLAG_TWO_KERNEL: producer kernel on stream A, consumer kernel on stream B
+    gated by cuStreamWaitValue32 on the first ready counter, every consumer unit polling its own counters.  Exact-mode
+    bits with H poisoned before every run, under delayed / reversed producers and every SM partition."""
+    kw = dict(kw)
+    kw["flags"] = kw.get("flags", 0) | TK
+    cfg = inputs.Config("two_kernel", 64, (1024, 4096, 1024), B.MLP_ACT_RELU, "exact", 5)
+    X, Ws, outs, _ = oracle_outs(cfg)
+    Xd, Wd = X.cuda(), [w.cuda() for w in Ws]
+    p = B.MlpPipe(cfg.M, cfg.widths, cfg.act, B.make_mode(P, **kw))
+    for _ in range(30):
+        p.poison_hidden(0x7FC0)
+        Y = p.run(Xd, Wd)
+        assert np.array_equal(inputs.as_u16(Y.cpu()), outs[-1])
+    st = p.stats()
+    assert st.ready_ok == 1 and st.status == 0 and st.runs == 30
+    assert st.units_done[0] == st.units[0] and st.units_done[1] == st.units[1]
+    assert 0 < st.producer_ctas < st.grid
+    p.close()
+
+
+def test_two_kernel_pipeline_on_baseline_configs():
+    """Same on BASELINE.json shapes, every element: cfg 0 (both distributions), cfg 1, cfg 2 and cfg 3 at full size."""
+    check(inputs.get_config(0, "exact"), B.make_mode(P, flags=TK))
+    check(inputs.get_config(0), B.make_mode(P, flags=TK))
+    for ci in (1, 2, 3):
+        check(inputs.CONFIGS[ci], B.make_mode(P, flags=TK))
+    with pytest.raises(B.MlpError) as e:
+        B.MlpPipe(128, inputs.CONFIGS[4].widths, 2, B.make_mode(P, flags=TK))     # a 4-layer chain: 2 layers only
+    assert e.value.status == B.MLP_ERR_UNSUPPORTED
+    with pytest.raises(B.MlpError):
+        B.MlpPipe(64, (64, 128, 128), 0, B.make_mode(S, flags=TK))
+
+
+@pytest.mark.parametrize("chunks,flags", [(2, 0), (4, 0), (2, B.MLP_FLAG_AUTOTUNE), (8, B.MLP_FLAG_AUTOTUNE)])
+def test_microbatch_coresident(chunks, flags):
+    """MLP_FLAG_MB_CORESIDENT: every micro-batch launch takes num_SMs / min(L, chunks) CTAs, so the launches of the two
+    streams run side by side (the overlap of PAPER.md:173).  Exact bits on cfg 0 and a 3-layer chain; autotuned too."""
+    f = flags | B.MLP_FLAG_MB_CORESIDENT
+    st = check(inputs.get_config(0, "exact"), B.make_mode(MB, chunks=chunks, flags=f))
+    assert st.grid <= 148 // 2
+    check(inputs.Config("mbc_3l", 96, (256, 1024, 512, 256), B.MLP_ACT_RELU, "exact", 9), B.make_mode(MB, chunks=chunks, flags=f))
+
+
+def test_microbatch_coresident_full_size():
+    for ci in (2, 3, 4):
+        check(inputs.CONFIGS[ci], B.make_mode(MB, chunks=2, flags=B.MLP_FLAG_MB_CORESIDENT | B.MLP_FLAG_AUTOTUNE))
+
+
+def test_single_kblock_mma_descriptor_probe():
+    """One layer, one output tile, ONE K-block (M = 16, K = 64, N = 128): the whole computation is the four tcgen05.mma
+    (128 x 16 x 16) of a single K-block, so a wrong bit in the shared-memory descriptor (start address, SBO, swizzle mode,
+    the +32 B K advance), in the instruction descriptor (M, N, formats, majors) or in the TMA box / swizzle shows up here
+    first and alone.  Inputs are chosen so that the output NAMES what was read: W[n, :] is a one-hot row selecting
+    k = (5 n + 3) mod 64 with weight 1 or 2, X[m, k] = ((7 m + 3 k) mod 5) - 2, hence Y[m, n] = w_n * X[m, k_n] -- and the
+    oracle agrees bit for bit (every value is a small integer)."""
+    M, K, N = 16, 64, 128
+    Xf = torch.tensor([[((7 * m + 3 * k) % 5) - 2 for k in range(K)] for m in range(M)], dtype=torch.float32)
+    Wf = torch.zeros((N, K), dtype=torch.float32)
+    for n in range(N):
+        Wf[n, (5 * n + 3) % K] = 1.0 + (n % 2)
+    X, W = Xf.to(torch.bfloat16), Wf.to(torch.bfloat16)
+    want, _ = oracle.mlp_chain(inputs.as_u16(X), [inputs.as_u16(W)], B.MLP_ACT_NONE)
+    expect = torch.stack([(1.0 + (n % 2)) * Xf[:, (5 * n + 3) % K] for n in range(N)], dim=1).to(torch.bfloat16)
+    assert np.array_equal(want[-1], inputs.as_u16(expect)), "the oracle must agree with the closed form of this probe"
+    for kind in (P, S):
+        p = B.MlpPipe(M, (K, N), B.MLP_ACT_NONE, B.make_mode(kind))
+        Y = p.run(X.cuda(), [W.cuda()])
+        torch.cuda.synchronize()
+        got = inputs.as_u16(Y.cpu())
+        if not np.array_equal(got, want[-1]):
+            bad = np.argwhere(got != want[-1])
+            m, n = bad[0]
+            raise AssertionError(f"{len(bad)} wrong elements; first at token {m}, feature {n} (K index {(5 * n + 3) % K}): "
+                                 f"got {oracle.u16_to_f64(got)[m, n]}, want {oracle.u16_to_f64(want[-1])[m, n]}")
+        p.close()
 
 
 def test_autotune_keeps_results_exact_and_state_consistent():
@@ -366,7 +479,7 @@ def test_workqueue_protocol_on_baseline_configs():
     check(inputs.CONFIGS[1], B.make_mode(P, flags=WQ))
     check(inputs.Config("wq_m320", 320, (256, 512, 256), 1, "exact", 3), B.make_mode(P, flags=WQ, split_k=2, tile_m=64))
     check(inputs.Config("wq_3l", 48, (256, 1024, 512, 256), B.MLP_ACT_RELU, "exact", 9), B.make_mode(P, flags=WQ))
-    err, st = sampled_rows_check(4, B.make_mode(P, flags=WQ), rows=[0, 31, 77, 127])
+    st = check(inputs.CONFIGS[4], B.make_mode(P, flags=WQ))   # full size, every element of Y and H_1..H_3
     assert st.n_layers == 4
 
 
@@ -475,9 +588,11 @@ def test_cta_pair_mode_exact(kw):
 
 
 def test_cta_pair_mode_full_size_and_protocol():
-    """Pair mode on full sizes (cfg 2: M = 256, sampled rows; cfg 4: the 4-layer chain) and under poison + delays."""
-    sampled_rows_check(2, B.make_mode(P, flags=PAIR), rows=[0, 1, 127, 128, 255])
-    err, st = sampled_rows_check(4, B.make_mode(P, flags=PAIR), rows=[0, 63, 64, 127])
+    """Pair mode on full sizes, every element (cfg 2: M = 256; cfg 3: the 70B shape; cfg 4: the 4-layer chain), and under
+    poison + delays."""
+    check(inputs.CONFIGS[2], B.make_mode(P, flags=PAIR))
+    check(inputs.CONFIGS[3], B.make_mode(P, flags=PAIR | B.MLP_FLAG_AUTOTUNE))
+    st = check(inputs.CONFIGS[4], B.make_mode(P, flags=PAIR))
     assert st.n_layers == 4
     cfg = inputs.Config("pair_adv", 64, (1024, 4096, 1024), B.MLP_ACT_RELU, "exact", 5)
     X, Ws, outs, _ = oracle_outs(cfg)
@@ -534,22 +649,30 @@ def test_many_m_blocks_rasterised_order(kw):
         assert st.units[0] >= 4 * 3
 
 
-def test_paper_shape_sampled_rows():
-    """The paper's own workload shape at its smallest M (2 layers, no activation, 8192 x 8192 weights,
-    M = 1024): sampled token rows against the oracle, CTA_PIPELINED with and without CTA pairs."""
-    cfg = inputs.Config("paper_1024", 1024, (8192, 8192, 8192), B.MLP_ACT_NONE, "normal", 7)
+@pytest.mark.parametrize("M", [1024, 4096])
+def test_paper_shape_sampled_rows(M):
+    """The paper's own workload shape (2 layers, no activation, 8192 x 8192 weights).  M = 4096 is
+    16 M-blocks = two rasterisation groups of 8 M-blocks (mlp_pipe.cu: build_table): token rows from EVERY 256-row M-block
+    (first, an inner and the last row of each) against the oracle, CTA_PIPELINED with and without CTA pairs and
+    SEQUENTIAL."""
+    cfg = inputs.Config(f"paper_{M}", M, (8192, 8192, 8192), B.MLP_ACT_NONE, "normal", 7)
     X, Ws = inputs.make_inputs(cfg)
-    rows = [0, 255, 256, 777, 1023]
+    rows = sorted(set(r for b in range(0, M, 256) for r in (b, b + 97 + (b // 256) % 64, b + 255)))
     outs, _ = oracle.mlp_chain(inputs.as_u16(X)[rows].copy(), [inputs.as_u16(w) for w in Ws], cfg.act)
-    for mode in (B.make_mode(P), B.make_mode(P, flags=PAIR)):
+    for mode in (B.make_mode(P), B.make_mode(P, flags=PAIR), B.make_mode(S)):
         got, hs, st = run_gpu(cfg, mode, X, Ws)
         assert st.status == 0 and st.ready_ok == 1
+        if M >= 2048:
+            assert st.tile_m == 256 and M // st.tile_m >= 16   # >= 2 rasterisation groups
+        e = oracle.rel_err(hs[0][rows], outs[0])
+        assert e["nan"] == 0 and e["err"] <= TOL, e
         e = oracle.rel_err(got[rows], outs[-1])
         assert e["nan"] == 0 and e["err"] <= TOL, e
+        assert not np.isnan(oracle.u16_to_f64(got)).any()
 
 
 def test_bench_custom_shape_line_is_well_formed():
-    """`bench.py --shape ... --pair` (the command behind profiles/paper_workload_r1d.md) on a small chain: one JSON line with the
+    """`bench.py --shape ... --pair` (the command behind profiles/paper_workload_r2.md) on a small chain: one JSON line with the
     contract's keys, a tensor- or HBM-bound roofline object and the in-build launch count."""
     import json
     import os
