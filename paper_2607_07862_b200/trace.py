@@ -27,6 +27,9 @@ def main() -> int:
     ap.add_argument("--workqueue", action="store_true")
     ap.add_argument("--pair", action="store_true", help="CTA pairs (MLP_FLAG_PAIR)")
     ap.add_argument("--every", type=int, default=12)
+    ap.add_argument("--split-k", type=str, default="")
+    ap.add_argument("--tile-n", type=int, default=0)
+    ap.add_argument("--act", type=int, default=-1, help="override the activation: 0 none, 1 ReLU, 2 GeLU-tanh")
     ap.add_argument("--sm-mhz", type=float, default=1965.0)
     args = ap.parse_args()
 
@@ -37,11 +40,14 @@ def main() -> int:
     from paper_2607_07862_b200 import inputs
 
     cfg = inputs.CONFIGS[args.config]
+    if args.act >= 0:
+        cfg = inputs.Config(cfg.name + f"_act{args.act}", cfg.M, cfg.widths, args.act, cfg.dist, cfg.seed)
     kind = B.MLP_CTA_PIPELINED if args.mode == "pipelined" else B.MLP_SEQUENTIAL
     flags = (0 if args.no_autotune else B.MLP_FLAG_AUTOTUNE) | (B.MLP_FLAG_WORKQUEUE if args.workqueue else 0) | (B.MLP_FLAG_PAIR if args.pair else 0)
     X, sets = bench.device_inputs(torch, cfg, bench.weight_sets_for(cfg))
     Y = torch.empty((cfg.M, cfg.widths[-1]), dtype=torch.bfloat16, device="cuda")
-    p = B.MlpPipe(cfg.M, cfg.widths, cfg.act, B.make_mode(kind, flags=flags))
+    split = [int(x) for x in args.split_k.split(",")] if args.split_k else []
+    p = B.MlpPipe(cfg.M, cfg.widths, cfg.act, B.make_mode(kind, flags=flags, split_k_layer=split, tile_n=args.tile_n))
     lat, _ = bench.time_steps(torch, p, X, sets, Y, 50, 10)
     st = p.stats()
     L = cfg.n_layers
@@ -62,7 +68,7 @@ def main() -> int:
             ts = " ".join(f"{(int(t) - t0) / 1e3:6.1f}" if t else "     -" for t in r.ts)
             w = [int(x) / cyc for x in r.wait]
             print(f"  cta {i:3d}: {ts} | waits: W ring {w[0]:5.1f}  MMA on operands {w[2]:5.1f}  epilogue on accumulator {w[4]:5.1f}  "
-                  f"flags {int(r.flag_stall_cycles) / cyc:5.1f}  gather {w[1]:4.1f}  partial {w[6]:4.1f}  direct {w[7]:4.1f} us")
+                  f"flags {int(r.flag_stall_cycles) / cyc:5.1f}  gather {w[1]:4.1f}  partial {w[6]:4.1f}  direct {w[7]:4.1f}  arrival {w[5]:4.1f} us")
             for u in range(B.MLP_UNIT_TRACE if hasattr(B, "MLP_UNIT_TRACE") else 12):
                 if r.unit_ts[u][0] == 0 or int(r.unit_ts[u][0]) < t0:
                     break

@@ -16,6 +16,7 @@ MODES = [
     dict(kind=P), dict(kind=S), dict(kind=MB, chunks=1), dict(kind=P, sm_split=0.5), dict(kind=P, split_k=4),
     dict(kind=P, split_k=3, flags=B.MLP_FLAG_DEBUG_REVERSE), dict(kind=P, tile_n=256, tile_m=64), dict(kind=P, tile_n=128),
     dict(kind=P, split_k_layer=[2, 9]), dict(kind=S, split_k=16), dict(kind=P, flags=B.MLP_FLAG_PAIR), dict(kind=S, flags=B.MLP_FLAG_PAIR, split_k=3),
+    dict(kind=MB, chunks=1, flags=B.MLP_FLAG_MB_CORESIDENT), dict(kind=P, flags=B.MLP_FLAG_TWO_KERNEL, sm_split=0.625),
 ]
 
 
@@ -84,6 +85,8 @@ def test_unit_tables_are_a_valid_schedule(M, widths, mode):
     if kw.get("tile_m") and kw["tile_m"] * 2 > 512:
         pytest.skip("shape not supported")
     pair = bool(kw.get("flags", 0) & B.MLP_FLAG_PAIR)
+    if kw.get("flags", 0) & B.MLP_FLAG_TWO_KERNEL and len(widths) != 3:
+        pytest.skip("the two-kernel pipeline is defined for 2 layers")
     if pair and (-(-min(M, 256) // 16) * 16) % 32 != 0 and M <= 256:
         pytest.skip("pair mode needs a token tile that is a multiple of 32")
     plan, tables = B.plan(M, widths, m, num_sms=148)
@@ -111,6 +114,27 @@ def test_pipelined_plan_orders_consumer_slices_by_k():
     if plan.split_k[1] > 4:
         first = tables[1][: plan.tiles[1]]
         assert all(u[2] == 0 and u[3] == 0 for u in first)
+
+
+def test_coresident_and_two_kernel_grids():
+    """MLP_FLAG_MB_CORESIDENT sizes every micro-batch launch so that the launches of the L streams fit on the device together;
+    MLP_FLAG_TWO_KERNEL partitions the SMs between the producer and the consumer kernel."""
+    cfg = inputs.CONFIGS[2]
+    full, _ = B.plan(cfg.M, cfg.widths, B.make_mode(MB, chunks=2), num_sms=148)
+    co, tco = B.plan(cfg.M, cfg.widths, B.make_mode(MB, chunks=2, flags=B.MLP_FLAG_MB_CORESIDENT), num_sms=148)
+    assert full.grid == 148 and co.grid == 74
+    co4, _ = B.plan(128, inputs.CONFIGS[4].widths, B.make_mode(MB, chunks=8, flags=B.MLP_FLAG_MB_CORESIDENT), num_sms=148)
+    assert co4.grid == 148 // 4            # four layers = four streams
+    tk, ttk = B.plan(cfg.M, cfg.widths, B.make_mode(P, flags=B.MLP_FLAG_TWO_KERNEL, sm_split=0.75), num_sms=148)
+    assert tk.grid == 148 and tk.producer_ctas == 148   # (per-kernel grids are 111 + 37; the plan reports the device-wide grid)
+    _check_tables(cfg.M, cfg.widths, tk, ttk)
+    import ctypes
+    out = B.mlp_plan()
+    w4 = (ctypes.c_int * 5)(*inputs.CONFIGS[4].widths)
+    bad = B.make_mode(S, flags=B.MLP_FLAG_TWO_KERNEL)
+    assert B.load().mlp_pipe_plan(128, 4, w4, ctypes.byref(bad), 148, ctypes.byref(out)) == B.MLP_ERR_UNSUPPORTED
+    bad = B.make_mode(P, flags=B.MLP_FLAG_MB_CORESIDENT)
+    assert B.load().mlp_pipe_plan(128, 4, w4, ctypes.byref(bad), 148, ctypes.byref(out)) == B.MLP_ERR_INVALID
 
 
 def test_plan_rejects_bad_arguments():
