@@ -357,6 +357,88 @@ __device__ __forceinline__ void store_chunk(const uint32_t (&v)[kC], int cc, flo
                     __uint_as_float(v[4 * g + 2]), __uint_as_float(v[4 * g + 3]));
 }
 
+// ---- direct epilogue in the MMA-fragment shape (steps a3 / a7).  The accumulator is feature-major (TMEM lane = feature,
+// column = token), the output token-major.  Read with tcgen05.ld.16x256b a thread holds, for one feature, PAIRS of
+// adjacent tokens -- exactly the register shape stmatrix.trans wants: act + cvt.rn.bf16x2 on the pair, then ONE
+// stmatrix.x4.trans per 16 lanes x 16 tokens writes 16 token rows of 16 features each into the staging buffer (the
+// transpose is done by the store unit, 512 bytes per instruction instead of 64 for a 2-byte st.shared per element: the
+// epilogue warps were bound by the number of load/store-unit instructions).  Token rows are kFragPitch bytes apart (256 + 16:
+// the 8 rows of a matrix then fall into different banks).  Leaves as 16-byte pieces exactly like emit_cols.
+constexpr uint32_t kFragPitch = kTileN * 2 + 16;
+static_assert(16 * kFragPitch <= kStageBufBytes, "16 token rows must fit a staging buffer");
+
+template <int kAct>
+__device__ __forceinline__ uint32_t frag_pack(uint32_t a, uint32_t b) {
+    float ya, yb;
+    if constexpr (kAct == kActGeluTanh) {
+        gelu_tanh_x2(__uint_as_float(a), __uint_as_float(b), ya, yb);
+    } else {
+        ya = act_apply<kAct>(__uint_as_float(a));
+        yb = act_apply<kAct>(__uint_as_float(b));
+    }
+    return pack_bf16x2(ya, yb);
+}
+
+template <int kAct>
+__device__ __forceinline__ void frag_stage(const uint32_t (&lo)[8], const uint32_t (&hi)[8], uint32_t row_addr) {
+    stmatrix_x4_trans(row_addr, frag_pack<kAct>(lo[0], lo[1]), frag_pack<kAct>(lo[2], lo[3]), frag_pack<kAct>(lo[4], lo[5]),
+                      frag_pack<kAct>(lo[6], lo[7]));
+    stmatrix_x4_trans(row_addr + 32u, frag_pack<kAct>(hi[0], hi[1]), frag_pack<kAct>(hi[2], hi[3]), frag_pack<kAct>(hi[4], hi[5]),
+                      frag_pack<kAct>(hi[6], hi[7]));
+}
+
+// taddr: this warp's lane quadrant, first column of the accumulator.  16 token columns per step; the loads of the next
+// step are in flight while the current one is converted and stored.
+__device__ __forceinline__ void drain_direct_frag(uint32_t taddr, int total, uint32_t bar_release, const EmitCtx& e, uint32_t& parity) {
+    const int begin = 0;
+    const int lane = e.r & 31, wq = e.r >> 5;
+    // stmatrix row address of this thread: matrix i = lane / 8 covers tokens 8 (i / 2) .. + 7 and features 8 (i % 2) .. + 7 of
+    // the 16-lane half; row j = lane % 8 is token 8 (i / 2) + j
+    const uint32_t row_off = static_cast<uint32_t>(((lane >> 4) * 8 + (lane & 7)) * kFragPitch + (wq * 32 + ((lane >> 3) & 1) * 8) * 2);
+    uint32_t la[8], ha[8], lb[8], hb[8];
+    tmem_ld_16x256b_x2(taddr + begin, la);
+    tmem_ld_16x256b_x2(taddr + (16u << 16) + begin, ha);
+    for (int cc = begin; cc < total; cc += 32) {
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {
+            const int c0 = cc + 16 * half;
+            if (c0 >= total) break;
+            tmem_ld_wait();
+            const bool more = c0 + 16 < total;
+            uint32_t (&lo)[8] = half == 0 ? la : lb;
+            uint32_t (&hi)[8] = half == 0 ? ha : hb;
+            uint32_t (&nlo)[8] = half == 0 ? lb : la;
+            uint32_t (&nhi)[8] = half == 0 ? hb : ha;
+            if (more) {
+                tmem_ld_16x256b_x2(taddr + c0 + 16, nlo);
+                tmem_ld_16x256b_x2(taddr + (16u << 16) + c0 + 16, nhi);
+            } else {
+                release_acc(bar_release);
+            }
+            const uint32_t buf = e.stage_s + (parity & 1u) * kStageBufBytes;
+            parity ^= 1u;
+            if (e.act == kActGeluTanh) frag_stage<kActGeluTanh>(lo, hi, buf + row_off);
+            else if (e.act == kActRelu) frag_stage<kActRelu>(lo, hi, buf + row_off);
+            else frag_stage<kActNone>(lo, hi, buf + row_off);
+            bar_sync(1, kEpiThreads);
+            const int rr = c0 >= e.tile_m ? 1 : 0, c = c0 - rr * e.tile_m;
+            const int n_base = e.n_first + rr * kTileN, m_first = e.m0 + c;
+            uint4 v[2];
+#pragma unroll
+            for (int p = 0; p < 2; ++p) {
+                const int piece = p * kEpiThreads + e.r;  // 16 pieces of 8 features per token row
+                v[p] = ld_shared_v4(buf + static_cast<uint32_t>(piece >> 4) * kFragPitch + static_cast<uint32_t>(piece & 15) * 16u);
+            }
+#pragma unroll
+            for (int p = 0; p < 2; ++p) {
+                const int piece = p * kEpiThreads + e.r;
+                const int m = m_first + (piece >> 4), n = n_base + (piece & 15) * 8;
+                if (m < e.m_end && n < e.N) *reinterpret_cast<uint4*>(e.out + static_cast<size_t>(m) * e.ld + n) = v[p];
+            }
+        }
+    }
+}
+
 // Drain one accumulator (`total` TMEM columns from taddr) in chunks of kC columns: the tcgen05.ld of the next
 // chunk is in flight while the current one is consumed -- kDirect: act + bf16 + transposed store of the output
 // (steps a3 / a7), else: fp32 split-K partial (step a8); once the last chunk has been read the accumulator is
@@ -1062,7 +1144,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 const long long te0 = clock64();
                 if (L.split == 1) {
                     const EmitCtx e{stage_s, r, L.out, out_row, nblk_c * tile_n, L.N, m0, P.m_end, L.act, tile_m};
-                    drain_acc<16, true>(taddr, static_cast<int>(acc_cols), (bar_tempty + 8 * acc) | (pair ? 1u : 0u), e, parity, nullptr);
+                    drain_direct_frag(taddr, static_cast<int>(acc_cols), (bar_tempty + 8 * acc) | (pair ? 1u : 0u), e, parity);
                     stored = true;
                     t_direct += static_cast<unsigned long long>(clock64() - te0);
                 } else {

@@ -244,6 +244,27 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
         : "r"(taddr)
         : "memory");
 }
+// TMEM -> registers in the MMA-fragment shape: 16 lanes x 16 columns per instruction; thread t holds, per group of 8
+// columns g, v[4g + 0..1] = (lane t / 4, columns 8g + 2 (t % 4) + {0, 1}) and v[4g + 2..3] = (lane t / 4 + 8, same columns)
+// (bit layout: cute/atom/copy_traits_sm100.hpp, SM100_TMEM_LOAD_16dp256b2x).  The lane field of taddr selects the first of
+// the 16 lanes (a multiple of 16 inside the warp's 32-lane quadrant).
+__device__ __forceinline__ void tmem_ld_16x256b_x2(uint32_t taddr, uint32_t (&v)[8]) {
+    asm volatile("tcgen05.ld.sync.aligned.16x256b.x2.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+                 : "r"(taddr)
+                 : "memory");
+}
+// Four 8 x 8 b16 matrices, registers -> shared memory, TRANSPOSED: register i of thread t holds (column t / 4, rows
+// 2 (t % 4) + {0, 1}) of matrix i; thread 8 i + j supplies the address of row j of matrix i (16 bytes per row).
+__device__ __forceinline__ void stmatrix_x4_trans(uint32_t row_addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+    asm volatile("stmatrix.sync.aligned.m8n8.x4.trans.shared.b16 [%0], {%1, %2, %3, %4};" ::"r"(row_addr), "r"(a), "r"(b), "r"(c), "r"(d)
+                 : "memory");
+}
+__device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {  // RNE both, lo in bits [0,16)
+    uint32_t d;
+    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
+    return d;
+}
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
 // named barrier among a subset of warps
