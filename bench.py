@@ -430,6 +430,18 @@ def per_config(torch, B, inputs, args, line):
         plan = {"grid": st.grid, "tile_m": st.tile_m, "tile_n": st.tile_n, "stages": st.stages, "split_k": list(st.split_k)[:cfg.n_layers]}
         entry["cta_pipelined"] = {"mean_us": lat["mean"], "median_us": lat["median"], "p10_us": lat["p10"], "p90_us": lat["p90"], "steps": steps}
         entry["plan"] = plan
+        # north_star's in-kernel evidence: stall-on-flag cycles (consumer prologue polling) and the producer / consumer split
+        entry["flag_stall_us_max_per_cta"] = int(st.flag_stall_cycles_max) / 1965.0
+        entry["units_per_layer"] = list(st.units)[:cfg.n_layers]
+        if ci == 2:   # BASELINE.json configs[2]: "sweep ... CTA_PIPELINED sm_split {1/4..3/4}"
+            sweep = {}
+            for sp in (0.25, 0.375, 0.5, 0.625, 0.75):
+                l2, s2 = measure(B.make_mode(B.MLP_CTA_PIPELINED, sm_split=sp, flags=tune))
+                sweep[str(sp)] = {"median_us": l2["median"], "producer_ctas": s2.producer_ctas,
+                                  "units_by_consumer_first_ctas": list(s2.units_by_consumer_ctas)[:cfg.n_layers],
+                                  "flag_stall_us_max_per_cta": int(s2.flag_stall_cycles_max) / 1965.0}
+            sweep["1.0"] = {"median_us": lat["median"], "producer_ctas": st.producer_ctas}
+            entry["sm_split_sweep"] = sweep
         entry["sequential_median_us"] = measure(B.make_mode(B.MLP_SEQUENTIAL, flags=tune))[0]["median"]
         entry["sequential_pdl_median_us"] = measure(B.make_mode(B.MLP_SEQUENTIAL, flags=tune | B.MLP_FLAG_PDL))[0]["median"]
         mbs = {}
