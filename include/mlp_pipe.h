@@ -165,11 +165,6 @@ typedef struct {
                         with undefined output and the handle reports MLP_ERR_TIMEOUT                   */
     int a_stages;    /* activation ring depth: 0 = as deep as the weight ring (the two rings then share their
                         barriers: one wait + one commit per K-block); another value gives the ring its own  */
-    int rows_layer[MLP_MAX_LAYERS]; /* weight rows (output features) per unit of layer l: 0 = auto, else a multiple of 8 in
-                        [64, tile_n].  The MMA is 128 rows high whatever this says; a lower tile only loads, and stores,
-                        fewer rows -- the way to cut a layer whose 128-row tiles fill a fraction of a wave (14336 rows =
-                        112 tiles on 148 SMs) into ceil(N / rows) tiles that occupy every SM.  Not with MLP_FLAG_PAIR /
-                        MLP_FLAG_WORKQUEUE (UNSUPPORTED).                                                         */
 } mlp_mode;
 
 /*
@@ -247,7 +242,6 @@ typedef struct {
     int tile_n;                                   /* resolved weight rows per unit (128 or 256)       */
     int reduce_mode[MLP_MAX_LAYERS];              /* how split tiles are summed: 0 not split, 1 by the
                                                      last-arriving slice, 2 by reduce units           */
-    int rows[MLP_MAX_LAYERS];                     /* resolved weight rows per unit of each layer      */
 } mlp_stats;
 int mlp_pipe_stats(mlp_pipe* h, mlp_stats* out, size_t bytes);
 
@@ -294,7 +288,6 @@ typedef struct {
     int ready_inc[MLP_MAX_LAYERS];   /* ready-counter increments per tile and run                         */
     int units[MLP_MAX_LAYERS];       /* tickets per layer                                                 */
     double model_us;                 /* planner's estimate of one run (device time, microseconds)         */
-    int rows[MLP_MAX_LAYERS];        /* weight rows per unit (tiles[l] = m_blks x ceil(N_l / rows[l]))     */
 } mlp_plan;
 typedef struct {
     uint16_t tile;     /* m_blk * n_blks + n_blk                                                          */

@@ -46,7 +46,6 @@ class mlp_mode(ctypes.Structure):
         ("stages", ctypes.c_int), ("kslice_tiles", ctypes.c_int), ("split_k", ctypes.c_int),
         ("flags", ctypes.c_uint), ("split_k_layer", ctypes.c_int * MLP_MAX_LAYERS),
         ("grid", ctypes.c_int), ("w_group", ctypes.c_int), ("timeout_ms", ctypes.c_int), ("a_stages", ctypes.c_int),
-        ("rows_layer", ctypes.c_int * MLP_MAX_LAYERS),
     ]
 
 
@@ -59,7 +58,7 @@ class mlp_stats(ctypes.Structure):
         ("flag_polls", ctypes.c_uint64), ("kernel_cycles_max", ctypes.c_uint64),
         ("units_done", ctypes.c_uint32 * MLP_MAX_LAYERS),
         ("units_by_consumer_ctas", ctypes.c_uint32 * MLP_MAX_LAYERS), ("ready_ok", ctypes.c_uint32),
-        ("tile_n", ctypes.c_int), ("reduce_mode", ctypes.c_int * MLP_MAX_LAYERS), ("rows", ctypes.c_int * MLP_MAX_LAYERS),
+        ("tile_n", ctypes.c_int), ("reduce_mode", ctypes.c_int * MLP_MAX_LAYERS),
     ]
 
 
@@ -78,7 +77,7 @@ class mlp_plan(ctypes.Structure):
         ("smem_bytes", ctypes.c_int),
         ("tiles", ctypes.c_int * MLP_MAX_LAYERS), ("split_k", ctypes.c_int * MLP_MAX_LAYERS),
         ("reduce_mode", ctypes.c_int * MLP_MAX_LAYERS), ("ready_inc", ctypes.c_int * MLP_MAX_LAYERS),
-        ("units", ctypes.c_int * MLP_MAX_LAYERS), ("model_us", ctypes.c_double), ("rows", ctypes.c_int * MLP_MAX_LAYERS),
+        ("units", ctypes.c_int * MLP_MAX_LAYERS), ("model_us", ctypes.c_double),
     ]
 
 
@@ -157,7 +156,7 @@ def _check(status: int, handle=None):
 
 def make_mode(kind: int = MLP_CTA_PIPELINED, chunks: int = 0, sm_split: float = 1.0, tile_m: int = 0, stages: int = 0,
               split_k: int = 0, split_k_layer: Sequence[int] = (), flags: int = 0, grid: int = 0,
-              timeout_ms: int = 0, w_group: int = 0, tile_n: int = 0, a_stages: int = 0, rows_layer: Sequence[int] = ()) -> mlp_mode:
+              timeout_ms: int = 0, w_group: int = 0, tile_n: int = 0, a_stages: int = 0) -> mlp_mode:
     m = mlp_mode()
     m.kind, m.chunks, m.sm_split, m.tile_m, m.stages = kind, chunks, sm_split, tile_m, stages
     m.tile_n = tile_n
@@ -166,8 +165,6 @@ def make_mode(kind: int = MLP_CTA_PIPELINED, chunks: int = 0, sm_split: float = 
     m.w_group = w_group
     for i, s in enumerate(split_k_layer):
         m.split_k_layer[i] = int(s)
-    for i, r in enumerate(rows_layer):
-        m.rows_layer[i] = int(r)
     return m
 
 

@@ -83,10 +83,7 @@ constexpr uint32_t kStatusFlagTimeout = 1u;
 struct LayerParams {
     int K, N;
     int kb_total;  // ceil(K / 64)
-    int rows;      // weight rows (= output features) per unit of this layer: a multiple of 8, <= 128 * n_sub (pair mode: 128 per
-                   // CTA).  Not necessarily 128 or 256: a layer whose 128-row tiles would fill only part of a wave (14336 rows =
-                   // 112 tiles on 148 SMs) is cut into ceil(N / rows) slightly lower tiles so that every SM streams
-    int n_blks;    // ceil(N / rows)
+    int n_blks;    // ceil(N / (128 * n_sub))
     int split;     // split of the contraction per output tile
     int units;     // entries of the unit table (MMA units + reduce units)
     int ticket_inc;  // what one launch adds to the ticket counter: units + CTAs arriving from the layer before
@@ -139,8 +136,7 @@ struct KernelParams {
     int layer_begin, layer_end;
     int m_off, m_end;  // token rows [m_off, m_end) of this launch
     int tile_m, m_blks;
-    int n_sub;          // 128-row MMAs per unit and K step (1 or 2): a unit covers up to 128 * n_sub weight rows (LayerParams::rows)
-    int w_slot_bytes;   // bytes of one weight stage of the ring = max over the layers of rows * 128 (a multiple of 1024)
+    int n_sub;          // 128-row MMAs per unit and K step (1 or 2): a unit covers 128 * n_sub weight rows
     int stages;         // weight ring depth
     int a_stages;       // activation ring depth
     int acc_stages;     // TMEM accumulators in the ring
@@ -543,7 +539,8 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
     const int nb_mul = pair ? 2 : 1;                       // 128-row counter tiles per table tile
     const int a_rows = pair ? tile_m / 2 : tile_m;         // token rows of the activation tile this CTA stages
     const int n_sub = P.n_sub;
-    const uint32_t w_tile_bytes = static_cast<uint32_t>(P.w_slot_bytes);  // one weight stage (the largest layer's rows x 128 B)
+    const int tile_n = kTileN * n_sub;  // weight rows per unit
+    const uint32_t w_tile_bytes = static_cast<uint32_t>(n_sub) * kWTileBytes;
     const uint32_t a_tile_bytes = static_cast<uint32_t>(a_rows) * (kTileK * 2);
     const int stages = P.stages;      // weight ring depth
     const int a_stages = P.a_stages;  // activation ring depth (= stages unless mlp_mode.a_stages asks otherwise)
@@ -638,12 +635,11 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
             const uint64_t pol = policy_evict_first();
             pre_w = static_cast<uint32_t>(min(stages, kb1 - kb0));
             my_stats->ts[3] = globaltimer_ns();
-            const int rows0 = P.layer[l0].rows;
             for (uint32_t i = 0; i < pre_w; ++i) {
-                mbar_arrive_expect_tx(bar_full + 8 * i, static_cast<uint32_t>(rows0) * (kTileK * 2));  // (the box is rows x 64 bf16)
+                mbar_arrive_expect_tx(bar_full + 8 * i, w_tile_bytes);
                 if (!(P.flags & kFlagNoEvictFirst))
-                    tma_load_2d_hint(smem_base + i * w_tile_bytes, &P.tm_w[l0], (kb0 + static_cast<int>(i)) * kTileK, n_blk * rows0, bar_full + 8 * i, pol);
-                else tma_load_2d(smem_base + i * w_tile_bytes, &P.tm_w[l0], (kb0 + static_cast<int>(i)) * kTileK, n_blk * rows0, bar_full + 8 * i);
+                    tma_load_2d_hint(smem_base + i * w_tile_bytes, &P.tm_w[l0], (kb0 + static_cast<int>(i)) * kTileK, n_blk * tile_n, bar_full + 8 * i, pol);
+                else tma_load_2d(smem_base + i * w_tile_bytes, &P.tm_w[l0], (kb0 + static_cast<int>(i)) * kTileK, n_blk * tile_n, bar_full + 8 * i);
             }
             if (l0 == P.layer_begin && !P.pdl_wait && !P.wait_first) {  // input of the launch: nothing to wait for
                 pre_a = static_cast<uint32_t>(min(min(a_stages, stages), kb1 - kb0));
@@ -805,9 +801,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                         // (pair mode: the counters are per 128-row block, tile_n = 128 here, and the acquire reaches the peer's
                         // loaders through the cluster-scope release / acquire of the slot hand-over: causality order is transitive)
                         const uint32_t* rd = Lp.ready + u.m_blk * Lp.n_blks * nb_mul;
-                        // producer tiles under this unit's K range: K-block kb reads columns [64 kb, 64 kb + 64) of the producer's
-                        // output, tile j of the producer wrote columns [j rows, (j + 1) rows)
-                        const int s0 = (u.kb0 * kTileK) / Lp.rows, s1 = min(Lp.n_blks * nb_mul, (u.kb1 * kTileK - 1) / Lp.rows + 1);
+                        const int s0 = (u.kb0 * kTileK) / tile_n, s1 = ((u.kb1 - 1) * kTileK) / tile_n + 1;
                         bool all = (s1 - s0) <= 256;  // (the scheduler runs a unit ahead: its round trips are off the critical path)
                         for (int sb = s0; sb < s1 && all; sb += 8) {
                             uint32_t v[8];
@@ -892,9 +886,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                     stage = pre % static_cast<uint32_t>(stages);
                     phase = pre / static_cast<uint32_t>(stages);
                 }
-                const int rows_u = P.layer[u.layer].rows;
-                const uint32_t w_box_bytes = static_cast<uint32_t>(rows_u) * (kTileK * 2);
-                const int w_row = pair ? (u.n_blk * 2 + static_cast<int>(rank)) * kTileN : u.n_blk * rows_u;
+                const int w_row = pair ? (u.n_blk * 2 + static_cast<int>(rank)) * kTileN : u.n_blk * tile_n;
                 while (kb < u.kb1) {
                     const int g = min(P.w_group, u.kb1 - kb);
                     uint32_t st = stage, ph = phase;
@@ -913,10 +905,10 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                             if (tell && i == 0) mbar_arrive(bar_wtaken + 8 * slot);
                             if (pair) {
                                 // each CTA loads its own 128 weight rows; the bytes of BOTH count on the leader's barrier
-                                if (leader) mbar_arrive_expect_tx(full, 2 * w_box_bytes);
+                                if (leader) mbar_arrive_expect_tx(full, 2 * w_tile_bytes);
                                 tma_load_2d_pair(dst, tm, kb * kTileK, w_row, full, pol);
                             } else {
-                                mbar_arrive_expect_tx(full, w_box_bytes);
+                                mbar_arrive_expect_tx(full, w_tile_bytes);
                                 if (hint) tma_load_2d_hint(dst, tm, kb * kTileK, w_row, full, pol);
                                 else tma_load_2d(dst, tm, kb * kTileK, w_row, full);
                             }
@@ -966,8 +958,8 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 // relaxed loads that are ISSUED a few K-blocks before their result is needed (the round trip
                 // overlaps the TMA issue of slices already known to be ready), then one acquire fence turns
                 // the observations into an acquire pattern (PTX memory model: relaxed read + fence.acq_rel).
-                const int slice_end = wait ? min(Lp.n_blks * nb_mul, (u.kb1 * kTileK - 1) / Lp.rows + 1) : 0;
-                int ready_upto = wait ? (u.kb0 * kTileK) / Lp.rows : 0;
+                const int slice_end = wait ? ((u.kb1 - 1) * kTileK) / tile_n + 1 : 0;
+                int ready_upto = wait ? (u.kb0 * kTileK) / tile_n : 0;
                 uint32_t v[8];
                 int pend_base = -1;  // >= 0: v[] holds in-flight reads of counters pend_base .. pend_base+7
                 int kb_first = u.kb0;
@@ -980,22 +972,14 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 for (int kb = kb_first; kb < u.kb1; ++kb) {
                     mbar_wait(bar_aempty + 8 * stage, phase ^ 1);
                     if (wait) {
-                        // last producer tile under this K-block's 64 columns (a K-block may straddle two tiles when the producer's
-                        // tiles are not multiples of 64 rows high)
-                        const int slice = min(slice_end - 1, (kb * kTileK + kTileK - 1) / Lp.rows);
+                        const int slice = (kb * kTileK) / tile_n;  // producer tile that wrote these columns
                         if (pend_base < 0 && ready_upto < slice_end && slice + 2 >= ready_upto) {
                             pend_base = ready_upto;
 #pragma unroll
                             for (int i = 0; i < 8; ++i)
                                 v[i] = (pend_base + i < slice_end) ? ((P.flags & kFlagAcquireLoads) ? ld_acquire_gpu(ready + pend_base + i) : ld_relaxed_gpu(ready + pend_base + i)) : target - 1u;
                         }
-                        while (slice >= ready_upto) {
-                            if (pend_base < 0) {  // (a second tile under the same K-block: another look)
-                                pend_base = ready_upto;
-#pragma unroll
-                                for (int i = 0; i < 8; ++i)
-                                    v[i] = (pend_base + i < slice_end) ? ((P.flags & kFlagAcquireLoads) ? ld_acquire_gpu(ready + pend_base + i) : ld_relaxed_gpu(ready + pend_base + i)) : target - 1u;
-                            }
+                        if (slice >= ready_upto) {
                             int n_ok = 0;
 #pragma unroll
                             for (int i = 0; i < 8; ++i)
@@ -1005,8 +989,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                                     const long long c0 = clock64();
                                     const uint64_t t0 = globaltimer_ns();
                                     uint32_t n = 0;
-                                    const uint32_t* ctr = ready + pend_base;  // the first tile not yet known to be published
-                                    while (static_cast<int32_t>(((P.flags & kFlagAcquireLoads) ? ld_acquire_gpu(ctr) : ld_relaxed_gpu(ctr)) - target) < 0) {
+                                    while (static_cast<int32_t>(((P.flags & kFlagAcquireLoads) ? ld_acquire_gpu(ready + slice) : ld_relaxed_gpu(ready + slice)) - target) < 0) {
                                         ++n;
                                         __nanosleep(32);
                                         if ((n & 255u) == 0) {
@@ -1077,9 +1060,6 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 ++mma_it;
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + acc * acc_cols;
-                // a second 128-row MMA per K step only where this layer's units are higher than 128 rows (rows 128 .. rows-1 of
-                // the stage; what lies beyond `rows` in the stage is stale and only produces accumulator rows that are never stored)
-                const bool two_blocks = !pair && P.layer[u.layer].rows > kTileN;
                 for (int kb = u.kb0; kb < u.kb1; ++kb) {
                     if (!unified) mbar_wait_timed(bar_afull + 8 * astage, aphase, wait_ops);
                     mbar_wait_timed(bar_full + 8 * stage, phase, wait_ops);
@@ -1093,7 +1073,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                         // [rr tile_m, (rr + 1) tile_m); both blocks read the same activation tile
                         const uint32_t accum = kb > u.kb0 ? 1u : 0u;
                         umma_bf16_kblock<pair>(d_tmem, a_lo, b_lo, desc_hi, idesc, accum);
-                        if (two_blocks) umma_bf16_kblock<false>(d_tmem + tile_m, a_lo + (kWTileBytes >> 4), b_lo, desc_hi, idesc, accum);
+                        if (!pair && n_sub == 2) umma_bf16_kblock<false>(d_tmem + tile_m, a_lo + (kWTileBytes >> 4), b_lo, desc_hi, idesc, accum);
                         if (pair) {  // the stages of BOTH CTAs are free again
                             umma_commit_pair(bar_empty + 8 * stage);
                             if (!unified) umma_commit_pair(bar_aempty + 8 * astage);
@@ -1139,11 +1119,6 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
             const int nblk_c = u.n_blk * nb_mul + static_cast<int>(rank);
             const int ctile = u.m_blk * (L.n_blks * nb_mul) + nblk_c;
             float* const ws_tile = L.ws + static_cast<size_t>(ctile) * L.split * ks_stride;
-            // this unit's features: [n_first, n_limit) -- L.rows of them (fewer in the layer's last tile), in blocks_u 128-row blocks
-            const int n_first = nblk_c * L.rows;
-            const int n_limit = min(L.N, n_first + L.rows);
-            const int blocks_u = (L.rows + kTileN - 1) / kTileN;
-            const int acc_used = blocks_u * tile_m;  // accumulator columns this layer's units fill
             bool stored = false;  // this unit wrote (part of) the layer's output
             int red_c0 = 0, red_c1 = 0;  // token columns of the tile whose partials this unit sums (none if equal)
             if (u.kind == kUnitReduce) {
@@ -1168,8 +1143,8 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                 if (it < kUnitTrace && r == 0) my_stats->unit_ts[it][2] = globaltimer_ns();
                 const long long te0 = clock64();
                 if (L.split == 1) {
-                    const EmitCtx e{stage_s, r, L.out, out_row, n_first, n_limit, m0, P.m_end, L.act, tile_m};
-                    drain_direct_frag(taddr, acc_used, (bar_tempty + 8 * acc) | (pair ? 1u : 0u), e, parity);
+                    const EmitCtx e{stage_s, r, L.out, out_row, nblk_c * tile_n, L.N, m0, P.m_end, L.act, tile_m};
+                    drain_direct_frag(taddr, static_cast<int>(acc_cols), (bar_tempty + 8 * acc) | (pair ? 1u : 0u), e, parity);
                     stored = true;
                     t_direct += static_cast<unsigned long long>(clock64() - te0);
                 } else {
@@ -1178,7 +1153,7 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
                     // (the columns of the n_sub blocks are consecutive both in TMEM and in the partial)
                     float* wsp = ws_tile + static_cast<size_t>(u.ks) * ks_stride + static_cast<size_t>(r) * 4;
                     const EmitCtx e{};
-                    drain_acc<16, false>(taddr, acc_used, (bar_tempty + 8 * acc) | (pair ? 1u : 0u), e, parity, wsp);
+                    drain_acc<16, false>(taddr, static_cast<int>(acc_cols), (bar_tempty + 8 * acc) | (pair ? 1u : 0u), e, parity, wsp);
                     // the 128 threads' partial stores happen-before thread 0's atomic (bar.sync); its release half
                     // is cumulative and publishes the CTA's whole partial, its acquire half (on the last arrival)
                     // makes the other slices' partials visible to the loads after the second barrier
@@ -1204,16 +1179,16 @@ __global__ void __launch_bounds__(kThreads, 1) mlp_pipe_kernel(const __grid_cons
             }
             if (red_c1 > red_c0) {
                 const long long tg0 = clock64();
-                for (int rr = 0; rr < blocks_u; ++rr) {
+                for (int rr = 0; rr < n_sub; ++rr) {
                     const float* blk = ws_tile + rr * blk_stride;
-                    const int n_base = n_first + rr * kTileN;
+                    const int n_base = nblk_c * tile_n + rr * kTileN;
                     for (int c = red_c0; c < red_c1; c += 16) {
                         float f[16];
                         uint32_t w[16];
                         gather16(blk, L.split, ks_stride, c, r, f);
 #pragma unroll
                         for (int j = 0; j < 16; ++j) w[j] = __float_as_uint(f[j]);
-                        emit_cols<16>(w, stage_s, parity, r, L.out, out_row, n_base, n_limit, m0 + c, P.m_end, L.act);
+                        emit_cols<16>(w, stage_s, parity, r, L.out, out_row, n_base, L.N, m0 + c, P.m_end, L.act);
                     }
                 }
                 t_gather += static_cast<unsigned long long>(clock64() - tg0);

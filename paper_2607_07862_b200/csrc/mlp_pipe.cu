@@ -57,8 +57,6 @@ struct mlp_pipe {
     std::vector<cudaStream_t> tk_stream;   // one stream per layer
     std::vector<cudaEvent_t> tk_done;      // one event per layer
     PFN_cuStreamWaitValue32_v11070 wait_value32 = nullptr;
-    int rows[kMaxLayers] = {0};   // weight rows per table tile of layer l (a multiple of 8, <= 128 * n_sub; pair mode: 256 per pair)
-    int w_slot = 0;               // bytes of one weight stage of the ring: the highest tile's rows x 128 B
     int split[kMaxLayers] = {0};
     int reduce_mode[kMaxLayers] = {0};
     int ready_inc[kMaxLayers] = {0};
@@ -190,13 +188,8 @@ int validate_mode(const mlp_mode& m, int M) {
         return MLP_ERR_UNSUPPORTED;
     if ((m.flags & MLP_FLAG_MB_CORESIDENT) && m.kind != MLP_MICROBATCH) return MLP_ERR_INVALID;
     if (m.stages < 0 || m.split_k < 0 || m.grid < 0 || m.timeout_ms < 0 || m.w_group < 0 || m.a_stages < 0) return MLP_ERR_INVALID;
-    for (int l = 0; l < kMaxLayers; ++l) {
+    for (int l = 0; l < kMaxLayers; ++l)
         if (m.split_k_layer[l] < 0) return MLP_ERR_INVALID;
-        if (m.rows_layer[l] < 0 || m.rows_layer[l] % 8 != 0) return MLP_ERR_INVALID;
-        if (m.rows_layer[l] != 0 && (m.rows_layer[l] < 64 || m.rows_layer[l] > 2 * kTileN || (m.flags & (MLP_FLAG_PAIR | MLP_FLAG_WORKQUEUE)) ||
-                                     (m.tile_n == kTileN && m.rows_layer[l] > kTileN)))
-            return MLP_ERR_UNSUPPORTED;
-    }
     if (m.tile_m > 256 || (m.tile_n != 0 && m.tile_n != kTileN && m.tile_n != 2 * kTileN) ||
         (m.tile_n == 2 * kTileN && m.tile_m > 256) || (m.tile_k != 0 && m.tile_k != kTileK) ||
         (m.kslice_tiles != 0 && m.kslice_tiles != 1))
@@ -420,7 +413,7 @@ struct Planner {
             const UnitDesc& d = h->table[l][w.idx];
             if (d.kind == kUnitReduce) return arrived[l][d.tile] == split_of(l) ? part_done[l][d.tile] : kInf;
             if (l == lb) return 0.0;
-            const int n_blks = h->tiles[l] / h->m_blks, n_prev = h->tiles[l - 1] / h->m_blks, tn = h->rows[l - 1];
+            const int n_blks = h->tiles[l] / h->m_blks, n_prev = h->tiles[l - 1] / h->m_blks, tn = kTileN * R;
             const int m_blk = d.tile / n_blks;
             const int j1 = std::min(n_prev - 1, ((d.b - 1) * kTileK) / tn);
             if (dep_j[wi] == 0) dep_j[wi] = (d.a * kTileK) / tn;
@@ -621,8 +614,6 @@ void resolve(mlp_pipe* h) {
     if (m.tile_n == 2 * kTileN) h->n_sub = 2;
     else if (m.tile_n == kTileN) h->n_sub = 1;
     else h->n_sub = wide_ok ? 2 : 1;
-    for (int l = 0; l < h->L; ++l)
-        if (m.rows_layer[l] > kTileN) h->n_sub = 2;
     // CTA pairs (MLP_FLAG_PAIR): a pair's unit is 256 weight rows x tile_m tokens, each CTA stages its own 128 rows and
     // HALF of the activation tile, and keeps a 128-row accumulator of tile_m columns -- n_sub = 1 per CTA
     h->pair = (m.flags & MLP_FLAG_PAIR) ? 1 : 0;
@@ -631,17 +622,7 @@ void resolve(mlp_pipe* h) {
     // Shared-memory rings: weight tiles (16 KB x n_sub each) and activation tiles (tile_m x 128 B each).
     // Weight ring depth: bytes in flight per SM just above the bandwidth-delay product (~80 KB x 148 SMs);
     // a deeper ring only lengthens the memory queues, and with them every flag / partial round trip.
-    // Tile heights.  Default: 128 * n_sub weight rows per unit.  mode.rows_layer[l] sets any multiple of 8 in [64, 128 * n_sub]:
-    // a layer whose full-height tiles fill only part of a wave (14336 rows = 112 tiles of 128 on 148 SMs) can be cut into
-    // ceil(N / rows) slightly lower tiles, so that every SM streams weights; the MMAs stay 128 rows high (the rows of the
-    // stage beyond `rows` are stale and give accumulator rows that are never stored).
-    int max_rows = 0;
-    for (int l = 0; l < h->L; ++l) {
-        h->rows[l] = h->pair ? 2 * kTileN : (m.rows_layer[l] > 0 ? std::min(m.rows_layer[l], kTileN * h->n_sub) : kTileN * h->n_sub);
-        max_rows = std::max(max_rows, h->pair ? kTileN : h->rows[l]);
-    }
-    const int w_tile = max_rows * kTileK * 2;   // one weight stage (per CTA)
-    h->w_slot = w_tile;
+    const int w_tile = h->n_sub * kWTileBytes;
     const int a_tile = (h->pair ? h->tile_m / 2 : h->tile_m) * kTileK * 2;
     const int max_smem = 227 * 1024 - kCtrlBytes - 1024 - kStageBytes;
     // (Measured on cfg 2, 16 KB weight + 32 KB activation tiles: 4 + 4 stages 82.4 us, 5 + 3 84.5, 6 + 3 86.5, 5 + 2 98.9 --
@@ -688,7 +669,7 @@ void resolve(mlp_pipe* h) {
     pl.force_tile_major = (m.flags & (MLP_FLAG_TILE_MAJOR | MLP_FLAG_DEBUG_REVERSE)) != 0 || h->two_kernel;
     for (int l = 0; l < h->L; ++l) {
         pl.kb_total[l] = ceil_div(h->widths[l], kTileK);
-        h->tiles[l] = ceil_div(h->widths[l + 1], h->rows[l]) * h->m_blks;
+        h->tiles[l] = ceil_div(h->widths[l + 1], kTileN * (h->pair ? 2 : h->n_sub)) * h->m_blks;
     }
     // smallest slice worth a unit: the fp32 partial of a split tile should stay below ~1/8 of the operand
     // bytes the slice streams
@@ -792,8 +773,7 @@ int build_base_params(mlp_pipe* h) {
         Lp.K = h->widths[l];
         Lp.N = h->widths[l + 1];
         Lp.kb_total = ceil_div(Lp.K, kTileK);
-        Lp.rows = h->pair ? kTileN : h->rows[l];      // rows per CTA and unit (pair mode: each CTA of the pair has 128)
-        Lp.n_blks = ceil_div(Lp.N, h->rows[l]);       // table tiles per M-block (pair mode: pairs of 128-row blocks)
+        Lp.n_blks = ceil_div(Lp.N, kTileN * (h->pair ? 2 : h->n_sub));  // table tiles per M-block (pair mode: pairs of 128-row blocks)
         Lp.split = h->split[l];
         Lp.units = static_cast<int>(h->table[l].size());
         Lp.act = l < h->L - 1 ? h->act : kActNone;
@@ -840,7 +820,6 @@ int build_base_params(mlp_pipe* h) {
     P.stages = h->stages;
     P.a_stages = h->a_stages;
     P.n_sub = h->n_sub;
-    P.w_slot_bytes = h->w_slot;
     P.pair = h->pair;
     {   // the next ticket is drawn ~2.5 loaded round trips (ticket atomic, table entry, ready counters) before
         // the weight loader runs out of K-blocks
@@ -977,8 +956,8 @@ int install_plan(mlp_pipe* h) {
         // The paper's data structures for every consumer layer l: groups g = (M-block, K-slice);
         // dependency array of producer tile (m, j) = the groups of M-block m whose K range covers the columns of j;
         // scoreboard[g] counts finished dependencies; the queue receives the units of a group when the count is full.
+        const int tn = kTileN * h->n_sub;
         for (int l = 1; l < h->L; ++l) {
-            const int tn = h->rows[l - 1];
             const int sp = h->split[l], n_blks = h->tiles[l] / h->m_blks, n_prev = h->tiles[l - 1] / h->m_blks;
             const int groups = h->m_blks * sp, units = static_cast<int>(h->table[l].size());
             if (units != h->tiles[l] * sp || units > 65535 || groups > 65535)
@@ -1056,7 +1035,7 @@ int create_impl(mlp_pipe** out, int M, int L, const int* widths, int dtype, int 
     h->num_sms = prop.multiProcessorCount;
     resolve(h);
     for (int l = 0; l < L; ++l) {  // the unit table stores tile ids and K-block bounds in 16 bits, the K-slice index in 8
-        const long long tiles128 = std::max<long long>(static_cast<long long>(ceil_div(widths[l + 1], kTileN)) * h->m_blks, h->tiles[l]);
+        const long long tiles128 = static_cast<long long>(ceil_div(widths[l + 1], kTileN)) * h->m_blks;
         if (tiles128 > 65535 || ceil_div(widths[l], kTileK) > 65535) {
             delete h;
             return fail(nullptr, MLP_ERR_UNSUPPORTED, "layer %d: %lld output tiles / %d K-blocks exceed the unit table's 16-bit fields", l,
@@ -1087,13 +1066,13 @@ int create_impl(mlp_pipe** out, int M, int L, const int* widths, int dtype, int 
     // counters are laid out for 128-row tiles (the larger count), so that the measured search may switch tile_n
     size_t words = 0;
     // (2 * ceil(N / 256) blocks per M-block: pair mode indexes a phantom block when N / 128 is odd)
-    for (int l = 0; l < L; ++l) words += 32 + 2 * static_cast<size_t>(round_up(std::max(2 * ceil_div(widths[l + 1], 2 * kTileN), ceil_div(widths[l + 1], 64)) * h->m_blks, 32));
+    for (int l = 0; l < L; ++l) words += 32 + 2 * static_cast<size_t>(round_up(2 * ceil_div(widths[l + 1], 2 * kTileN) * h->m_blks, 32));
     h->counters_words = words;
     CREATE_TRY(cudaMalloc(&h->counters, words * sizeof(uint32_t)));
     {
         uint32_t* p = h->counters;
         for (int l = 0; l < L; ++l) {
-            const int t128 = round_up(std::max(2 * ceil_div(widths[l + 1], 2 * kTileN), ceil_div(widths[l + 1], 64)) * h->m_blks, 32);
+            const int t128 = round_up(2 * ceil_div(widths[l + 1], 2 * kTileN) * h->m_blks, 32);
             h->ticket[l] = p;  // own 128-byte line
             p += 32;
             h->arrive[l] = p;
@@ -1180,7 +1159,7 @@ int run_core(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStre
     }
     if ((rc = lookup_tmap(h, h->cache_x, &h->cache_x_next, X, h->M, h->widths[0], h->pair ? h->tile_m / 2 : h->tile_m, &P.tm_a[0]))) return rc;
     for (int l = 0; l < h->L; ++l)
-        if ((rc = lookup_tmap(h, h->cache_w[l], &h->cache_w_next[l], W[l], h->widths[l + 1], h->widths[l], h->pair ? kTileN : h->rows[l], &P.tm_w[l])))
+        if ((rc = lookup_tmap(h, h->cache_w[l], &h->cache_w_next[l], W[l], h->widths[l + 1], h->widths[l], kTileN * h->n_sub, &P.tm_w[l])))
             return rc;
     P.layer[h->L - 1].out = static_cast<__nv_bfloat16*>(Y);
 
@@ -1549,7 +1528,6 @@ int mlp_pipe_stats(mlp_pipe* h, mlp_stats* out, size_t bytes) {
     st.stages = h->stages;
     st.tile_m = h->tile_m;
     st.tile_n = kTileN * (h->pair ? 2 : h->n_sub);
-    for (int l = 0; l < h->L; ++l) st.rows[l] = h->rows[l];
     st.producer_ctas = h->two_kernel ? h->lgrid[0] : h->producer_ctas;
     for (int l = 0; l < h->L; ++l) {
         st.split_k[l] = h->split[l];
@@ -1662,9 +1640,7 @@ void mlp_pipe_destroy(mlp_pipe* h) {
 
 static bool fits_unit_table(const mlp_pipe& h) {
     for (int l = 0; l < h.L; ++l)
-        if (std::max<long long>(static_cast<long long>(ceil_div(h.widths[l + 1], kTileN)) * h.m_blks, h.tiles[l]) > 65535 ||
-            ceil_div(h.widths[l], kTileK) > 65535)
-            return false;
+        if (static_cast<long long>(ceil_div(h.widths[l + 1], kTileN)) * h.m_blks > 65535 || ceil_div(h.widths[l], kTileK) > 65535) return false;
     return true;
 }
 
@@ -1703,7 +1679,6 @@ int mlp_pipe_plan(int M, int n_layers, const int* widths, const mlp_mode* mode, 
         out->reduce_mode[l] = h.reduce_mode[l];
         out->ready_inc[l] = h.ready_inc[l];
         out->units[l] = static_cast<int>(h.table[l].size());
-        out->rows[l] = h.rows[l];
     }
     return MLP_OK;
 }

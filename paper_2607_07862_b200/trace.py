@@ -29,8 +29,6 @@ def main() -> int:
     ap.add_argument("--every", type=int, default=12)
     ap.add_argument("--split-k", type=str, default="")
     ap.add_argument("--tile-n", type=int, default=0)
-    ap.add_argument("--rows", type=str, default="", help="weight rows per unit, comma list per layer (mlp_mode.rows_layer)")
-    ap.add_argument("--stages", type=int, default=0)
     ap.add_argument("--act", type=int, default=-1, help="override the activation: 0 none, 1 ReLU, 2 GeLU-tanh")
     ap.add_argument("--sm-mhz", type=float, default=1965.0)
     args = ap.parse_args()
@@ -49,8 +47,7 @@ def main() -> int:
     X, sets = bench.device_inputs(torch, cfg, bench.weight_sets_for(cfg))
     Y = torch.empty((cfg.M, cfg.widths[-1]), dtype=torch.bfloat16, device="cuda")
     split = [int(x) for x in args.split_k.split(",")] if args.split_k else []
-    p = B.MlpPipe(cfg.M, cfg.widths, cfg.act, B.make_mode(kind, flags=flags, split_k_layer=split, tile_n=args.tile_n,
-                                                              rows_layer=[int(x) for x in args.rows.split(",")] if args.rows else [], stages=args.stages))
+    p = B.MlpPipe(cfg.M, cfg.widths, cfg.act, B.make_mode(kind, flags=flags, split_k_layer=split, tile_n=args.tile_n))
     lat, _ = bench.time_steps(torch, p, X, sets, Y, 50, 10)
     st = p.stats()
     L = cfg.n_layers

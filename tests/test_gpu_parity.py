@@ -309,54 +309,6 @@ def test_two_pipelined_handles_on_two_streams():
         ps[k].close()
 
 
-ROWS_CASES = [
-    # (M, widths, act, mode kwargs): tile heights that are not 128 / 256 -- lower than 128 (a consumer K-block then straddles two
-    # producer tiles), between 128 and 256 (second MMA block partly stale), ragged last tiles, with and without K-splits
-    (64, (512, 2048, 512), 1, dict(rows_layer=[104, 72])),
-    (64, (512, 2048, 512), 1, dict(rows_layer=[72, 104], split_k_layer=[1, 4])),
-    (64, (512, 2048, 512), 1, dict(rows_layer=[200, 168], split_k_layer=[2, 3])),
-    (96, (520, 1544, 776), 1, dict(rows_layer=[88, 248])),
-    (130, (264, 392, 200), 1, dict(rows_layer=[64, 120], split_k=2)),
-    (300, (136, 264, 136), 1, dict(rows_layer=[136, 72])),
-    (48, (256, 1024, 512, 256), 1, dict(rows_layer=[96, 176, 80], split_k_layer=[1, 2, 1])),
-    (16, (64, 128, 128), 1, dict(rows_layer=[64, 64])),
-]
-
-
-@pytest.mark.parametrize("M,widths,act,kw", ROWS_CASES, ids=[str(i) for i in range(len(ROWS_CASES))])
-@pytest.mark.parametrize("kind", [P, S])
-def test_tile_heights_exact(M, widths, act, kw, kind):
-    """mlp_mode.rows_layer: units that are not 128 or 256 weight rows high (any multiple of 8 from 64).  Integer inputs:
-    H_l and Y must equal the oracle bit for bit in CTA_PIPELINED (ready counters per odd-height producer tile, consumer
-    K-blocks straddling two of them) and SEQUENTIAL, H poisoned first."""
-    cfg = inputs.Config(f"rows_{M}_{'_'.join(map(str, widths))}", M, widths, act, "exact", 17)
-    st = check(cfg, B.make_mode(kind, **kw))
-    assert list(st.rows)[:cfg.n_layers] == list(kw["rows_layer"])
-
-
-def test_tile_heights_full_size_and_protocol():
-    """Odd tile heights on BASELINE.json shapes at full size, every element (cfg 3: 144 + 147 units instead of 112 + 128;
-    cfg 4 and cfg 2: 138-unit producer layers), and under delayed producers with H poisoned before every run."""
-    check(inputs.CONFIGS[3], B.make_mode(P, rows_layer=[200, 168], split_k_layer=[1, 3], stages=5))
-    check(inputs.CONFIGS[4], B.make_mode(P, rows_layer=[104, 0, 104, 0], flags=B.MLP_FLAG_AUTOTUNE))
-    check(inputs.CONFIGS[2], B.make_mode(P, rows_layer=[104, 0]))
-    check(inputs.CONFIGS[1], B.make_mode(P, rows_layer=[104, 112]))
-    cfg = inputs.Config("rows_adv", 64, (1024, 4096, 1024), B.MLP_ACT_RELU, "exact", 5)
-    X, Ws, outs, _ = oracle_outs(cfg)
-    Xd, Wd = X.cuda(), [w.cuda() for w in Ws]
-    p = B.MlpPipe(cfg.M, cfg.widths, cfg.act, B.make_mode(P, rows_layer=[88, 72], split_k=4, flags=B.MLP_FLAG_DEBUG_DELAY))
-    for _ in range(30):
-        p.poison_hidden(0x7FC0)
-        Y = p.run(Xd, Wd)
-        assert np.array_equal(inputs.as_u16(Y.cpu()), outs[-1])
-    st = p.stats()
-    assert st.ready_ok == 1 and st.status == 0 and st.runs == 30
-    p.close()
-    with pytest.raises(B.MlpError) as e:
-        B.MlpPipe(64, (512, 2048, 512), 1, B.make_mode(P, rows_layer=[104, 72], flags=PAIR))
-    assert e.value.status == B.MLP_ERR_UNSUPPORTED
-
-
 TK = B.MLP_FLAG_TWO_KERNEL
 
 

@@ -17,7 +17,6 @@ MODES = [
     dict(kind=P, split_k=3, flags=B.MLP_FLAG_DEBUG_REVERSE), dict(kind=P, tile_n=256, tile_m=64), dict(kind=P, tile_n=128),
     dict(kind=P, split_k_layer=[2, 9]), dict(kind=S, split_k=16), dict(kind=P, flags=B.MLP_FLAG_PAIR), dict(kind=S, flags=B.MLP_FLAG_PAIR, split_k=3),
     dict(kind=MB, chunks=1, flags=B.MLP_FLAG_MB_CORESIDENT), dict(kind=P, flags=B.MLP_FLAG_TWO_KERNEL, sm_split=0.625),
-    dict(kind=P, rows_layer=[104, 72, 200, 64]), dict(kind=S, rows_layer=[200, 168], split_k_layer=[1, 3]),
 ]
 
 
@@ -34,8 +33,7 @@ def _check_tables(M, widths, plan, tables, pair=False):
     for l in range(L):
         K, N = widths[l], widths[l + 1]
         kb_total = -(-K // 64)
-        assert plan.rows[l] % 8 == 0 and 64 <= plan.rows[l] <= plan.tile_n
-        tiles = plan.m_blks * -(-N // plan.rows[l])
+        tiles = plan.m_blks * -(-N // plan.tile_n)
         assert plan.tiles[l] == tiles
         sp = plan.split_k[l]
         table = tables[l]
