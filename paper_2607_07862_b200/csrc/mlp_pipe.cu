@@ -1024,6 +1024,9 @@ int create_impl(mlp_pipe** out, int M, int L, const int* widths, int dtype, int 
     if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return fail(nullptr, MLP_ERR_UNSUPPORTED, "no CUDA device");
     if (prop.major != 10) return fail(nullptr, MLP_ERR_UNSUPPORTED, "device is sm_%d%d, this library is sm_100a only", prop.major, prop.minor);
 
+    for (int l = 0; l < L; ++l)  // cheap bound before the planner runs: even 256 x 256 tiles would overflow the unit table
+        if (static_cast<long long>(ceil_div(M, 256)) * ceil_div(widths[l + 1], 2 * kTileN) > 65535 || ceil_div(widths[l], kTileK) > 65535)
+            return fail(nullptr, MLP_ERR_UNSUPPORTED, "layer %d exceeds the unit table's 16-bit tile / K-block fields", l);
     mlp_pipe* h = new (std::nothrow) mlp_pipe();
     if (!h) return fail(nullptr, MLP_ERR_OOM, "host allocation failed");
     h->M = M;
@@ -1659,7 +1662,9 @@ int mlp_pipe_plan(int M, int n_layers, const int* widths, const mlp_mode* mode, 
     for (int l = 0; l <= n_layers; ++l) h.widths[l] = widths[l];
     h.mode = m;
     h.num_sms = num_sms;
-    if (M > 256 * 65535) return MLP_ERR_UNSUPPORTED;
+    for (int l = 0; l < n_layers; ++l)
+        if (static_cast<long long>(ceil_div(M, 256)) * ceil_div(widths[l + 1], 2 * kTileN) > 65535 || ceil_div(widths[l], kTileK) > 65535)
+            return MLP_ERR_UNSUPPORTED;
     resolve(&h);
     if (!fits_unit_table(h)) return MLP_ERR_UNSUPPORTED;
     memset(out, 0, sizeof *out);
@@ -1701,7 +1706,9 @@ int mlp_pipe_plan_units(int M, int n_layers, const int* widths, const mlp_mode* 
     for (int l = 0; l <= n_layers; ++l) h.widths[l] = widths[l];
     h.mode = m;
     h.num_sms = num_sms;
-    if (M > 256 * 65535) return MLP_ERR_UNSUPPORTED;
+    for (int l = 0; l < n_layers; ++l)
+        if (static_cast<long long>(ceil_div(M, 256)) * ceil_div(widths[l + 1], 2 * kTileN) > 65535 || ceil_div(widths[l], kTileK) > 65535)
+            return MLP_ERR_UNSUPPORTED;
     resolve(&h);
     if (!fits_unit_table(h)) return MLP_ERR_UNSUPPORTED;
     const std::vector<UnitDesc>& t = h.table[layer];

@@ -148,3 +148,8 @@ def test_plan_rejects_bad_arguments():
     bad = (ctypes.c_int * 3)(64, 100, 128)
     assert lib.mlp_pipe_plan(16, 2, bad, None, 148, ctypes.byref(out)) == B.MLP_ERR_INVALID
     assert lib.mlp_pipe_plan(16, 2, w, None, 148, ctypes.byref(out)) == B.MLP_OK
+    # limits of the unit table's 16-bit fields: rejected before the planner runs (include/mlp_pipe.h, "limits")
+    huge = (ctypes.c_int * 3)(64, 1 << 20, 128)
+    assert lib.mlp_pipe_plan(1 << 20, 2, huge, None, 148, ctypes.byref(out)) == B.MLP_ERR_UNSUPPORTED
+    deep = (ctypes.c_int * 3)(64 * 65536, 128, 128)
+    assert lib.mlp_pipe_plan(16, 2, deep, None, 148, ctypes.byref(out)) == B.MLP_ERR_UNSUPPORTED
