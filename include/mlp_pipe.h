@@ -301,6 +301,49 @@ int mlp_pipe_plan(int M, int n_layers, const int* widths, const mlp_mode* mode, 
 int mlp_pipe_plan_units(int M, int n_layers, const int* widths, const mlp_mode* mode, int num_sms, int layer,
                         mlp_unit* out, int max_units, int* n_out);
 
+/*
+ * The same CTA-pipelined pass (one persistent launch, plan of a default CTA_PIPELINED handle) for
+ * callers that cannot let this library allocate -- no handle, no cudaMalloc, no cudaFree, no pinned-memory or
+ * stream / event creation, on the first call or on any later one.
+ *
+ * Who needs this.  mlp_pipe_create reserves the hidden activations, the split-K partials, the tickets and counters and
+ * the unit tables with cudaMalloc.  Two kinds of caller cannot afford that: a serving process whose own memory manager
+ * has already claimed the free HBM at start-up (KV-cache pools and the like), where a later cudaMalloc fails or eats into
+ * a budget the library knows nothing about; and a decode loop that shares the GPU with other streams, where a
+ * cudaMalloc / cudaFree in the middle of the loop can stall the whole device, not just the calling stream.  For them all of
+ * that scratch lives in one fixed array of MLP_STATIC_SCRATCH_BYTES that is part of the library image: every GPU on which
+ * the library runs a kernel holds these 32 MiB from the moment the library's code is loaded there until the process
+ * exits, whether or not this function is ever called.
+ *
+ * Arguments: M tokens; widths[0..n_layers] = K, N_1, .., N_L (host pointer, 1 <= n_layers <= MLP_MAX_LAYERS); act as for
+ * mlp_pipe_create; X [M x K], W[l] [N_{l+1} x N_l] (W = host array of n_layers DEVICE pointers), Y [M x N_L]: device
+ * pointers owned by the caller, layouts and alignment as above; cuda_stream as for mlp_pipe_run.  Asynchronous: clears
+ * the part of the array that must start at zero, sends the unit tables and launches, all on the caller's stream, and
+ * returns.  Y is fully overwritten; plan and kernel are those of a handle created with mode == NULL, and so is the result.
+ *
+ * Limit: the plan's scratch (sum over layers of M x N_l x 2 bytes of hidden activations + tiles x split x tile bytes of
+ * fp32 partials + a few hundred KB of counters, tables and records) must fit MLP_STATIC_SCRATCH_BYTES; all five
+ * BASELINE.json configs do (the 4-layer chain needs about 24 MiB).  A larger problem is rejected with
+ * MLP_ERR_UNSUPPORTED before anything is enqueued, and mlp_pipe_last_error(NULL) names the bytes it would have needed.
+ *
+ * Set-up: the FIRST call on each device looks up where that device keeps the array (a symbol look-up, which may load
+ * the library's device code) with that device current; make that first call during start-up, before any stream capture
+ * begins.  The first call for a new shape also plans it on the host (tens of milliseconds for the large configs); calls
+ * that repeat the previous shape reuse that plan.
+ *
+ * Sharing: there is ONE array per device and every call uses it, whatever its shape, and finds in it what the call
+ * before left behind.  Calls must therefore not overlap on the GPU: order them on one stream, or with events.  Two calls
+ * in flight at once (two streams, two threads) clear and overwrite each other's counters and activations -- wrong output,
+ * or CTAs that wait until the watchdog (2 s) lets them go.  Handles made by mlp_pipe_create have their own memory and may
+ * run alongside.  This entry point keeps no pinned status mirror, so it cannot report a watchdog expiry; it returns only
+ * what can be known at enqueue time.
+ * Errors: INVALID (null / misaligned pointer, bad dims or act), UNSUPPORTED (no sm_100 device, scratch limit, unit-table
+ * limits), CUDA (symbol look-up, memset, copy or launch failure).  Messages: mlp_pipe_last_error(NULL).
+ */
+#define MLP_STATIC_SCRATCH_BYTES (32u << 20)
+int mlp_pipe_run_static(int M, int n_layers, const int* widths, int act, const void* X, const void* const* W, void* Y,
+                        void* cuda_stream);
+
 /* Free everything the handle owns (synchronises the device).  NULL is ignored. */
 void mlp_pipe_destroy(mlp_pipe* h);
 

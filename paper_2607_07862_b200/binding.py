@@ -36,7 +36,9 @@ EXPORTS = [
     "mlp_pipe_create", "mlp_pipe_create_chain", "mlp_pipe_run", "mlp_pipe_run_chain", "mlp_pipe_run_host",
     "mlp_pipe_hidden", "mlp_pipe_poison_hidden", "mlp_pipe_stats", "mlp_pipe_destroy", "mlp_status_string",
     "mlp_pipe_last_error", "mlp_pipe_version", "mlp_pipe_cta_records", "mlp_pipe_plan", "mlp_pipe_plan_units",
+    "mlp_pipe_run_static",
 ]
+MLP_STATIC_SCRATCH_BYTES = 32 << 20
 
 
 class mlp_mode(ctypes.Structure):
@@ -129,6 +131,8 @@ def load(build_if_missing: bool = True):
     lib.mlp_pipe_plan_units.restype = ci
     lib.mlp_pipe_plan_units.argtypes = [ci, ci, ctypes.POINTER(ci), ctypes.POINTER(mlp_mode), ci, ci, ctypes.POINTER(mlp_unit), ci,
                                         ctypes.POINTER(ci)]
+    lib.mlp_pipe_run_static.restype = ci
+    lib.mlp_pipe_run_static.argtypes = [ci, ci, ctypes.POINTER(ci), ci, vp, ctypes.POINTER(vp), vp, vp]
     lib.mlp_pipe_destroy.restype = None
     lib.mlp_pipe_destroy.argtypes = [vp]
     lib.mlp_status_string.restype = ctypes.c_char_p
@@ -273,6 +277,29 @@ class _RawCudaBuffer:
 
     def __init__(self, ptr: int, nbytes: int):
         self.__cuda_array_interface__ = {"shape": (nbytes,), "typestr": "|u1", "data": (ptr, False), "version": 2}
+
+
+def run_static(X: torch.Tensor, Ws: Sequence[torch.Tensor], act: int, Y: Optional[torch.Tensor] = None,
+               stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """mlp_pipe_run_static: the CTA-pipelined pass without a handle, for callers that must not allocate device memory.
+
+    The library side allocates nothing: its scratch is a fixed MLP_STATIC_SCRATCH_BYTES array inside the library, shared
+    by every call on the device (so calls must not overlap on the GPU; see include/mlp_pipe.h).  Pass `Y` to keep this
+    wrapper from allocating the output tensor through torch.
+    """
+    if not torch.cuda.is_available():
+        raise RuntimeError("mlp_pipe needs a CUDA device (sm_100a); there is no CPU fallback")
+    lib = load()
+    M, widths = int(X.shape[0]), [int(X.shape[1])] + [int(w.shape[0]) for w in Ws]
+    L = len(Ws)
+    if Y is None:
+        Y = torch.empty((M, widths[-1]), dtype=torch.bfloat16, device=X.device)
+    xp = _dev_ptr(X, (M, widths[0]), "X")
+    yp = _dev_ptr(Y, (M, widths[-1]), "Y")
+    wp = (ctypes.c_void_p * L)(*[_dev_ptr(w, (widths[l + 1], widths[l]), f"W[{l}]") for l, w in enumerate(Ws)])
+    wd = (ctypes.c_int * (L + 1))(*widths)
+    _check(lib.mlp_pipe_run_static(M, L, wd, int(act), xp, wp, yp, _stream_ptr(stream)), None)
+    return Y
 
 
 def plan(M: int, widths: Sequence[int], mode: Optional[mlp_mode] = None, num_sms: int = 148):

@@ -1741,3 +1741,210 @@ const char* mlp_pipe_last_error(const mlp_pipe* h) { return h ? h->last_error.c_
 const char* mlp_pipe_version(void) { return "mlp_pipe 0.1 sm_100a tcgen05/TMA bf16 (CTA-pipelined chained GEMM)"; }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// mlp_pipe_run_static (include/mlp_pipe.h): the CTA-pipelined pass for callers that must not
+// allocate.  Same kernel, same planner, same launch as a default CTA_PIPELINED handle -- but
+// everything the kernel needs beyond X, W_l and Y (hidden activations, split-K partials, tickets
+// and counters, unit tables, per-CTA records) lives in ONE fixed array that is part of the
+// library image, instead of in cudaMalloc'ed buffers owned by a handle.
+//
+// The array below is device memory, but in HOST code its name only stands for it: taking its
+// address on the host does not give a device pointer.  The device address is looked up once per
+// device with cudaGetSymbolAddress (static_slot_for_current_device) and only that pointer is
+// handed to the kernel.
+// ---------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_static_scratch[MLP_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+constexpr size_t kStaticAlign = 256;
+
+struct StaticSlot {
+    unsigned char* base = nullptr;  // this device's copy of g_static_scratch (from cudaGetSymbolAddress)
+    int num_sms = 0;
+    mlp_pipe* plan = nullptr;       // host-side launch plan of the most recent shape; its device pointers point into `base`
+    size_t zero_bytes = 0;          // the head of the array (tickets, counters, epoch, status, per-CTA records): cleared per call
+};
+
+std::mutex g_static_mutex;          // calls are serialised on the host; on the GPU the caller's streams order them
+StaticSlot g_static_slot[kStaticMaxDevices];
+
+size_t static_align_up(size_t v) { return (v + kStaticAlign - 1) / kStaticAlign * kStaticAlign; }
+
+// First call on a device: find where that device keeps the array.  The device must be current.
+int static_slot_for_current_device(StaticSlot** out) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return fail(nullptr, MLP_ERR_UNSUPPORTED, "no CUDA device");
+    if (dev < 0 || dev >= kStaticMaxDevices) return fail(nullptr, MLP_ERR_UNSUPPORTED, "device ordinal %d is beyond the %d this entry point keeps state for", dev, kStaticMaxDevices);
+    StaticSlot& S = g_static_slot[dev];
+    if (!S.base) {
+        int major = 0, sms = 0;
+        if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+            return fail(nullptr, MLP_ERR_UNSUPPORTED, "no CUDA device");
+        if (major != 10) return fail(nullptr, MLP_ERR_UNSUPPORTED, "device is sm_%dx, this library is sm_100a only", major);
+        unsigned char* p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(reinterpret_cast<void**>(&p), g_static_scratch);
+        if (e != cudaSuccess || !p) {
+            cudaGetLastError();
+            return fail(nullptr, MLP_ERR_CUDA, "cudaGetSymbolAddress(g_static_scratch): %s", cudaGetErrorString(e));
+        }
+        if (reinterpret_cast<uintptr_t>(p) % kStaticAlign) return fail(nullptr, MLP_ERR_CUDA, "static scratch array is not %zu-byte aligned", kStaticAlign);
+        S.base = p;
+        S.num_sms = sms;
+    }
+    *out = &S;
+    return MLP_OK;
+}
+
+// Lay the plan's device buffers out inside the array: [cleared per call: tickets + arrival + ready counters | epoch |
+// status | per-CTA records] [unit tables] [hidden activations] [split-K partials].  With base == nullptr only the sizes
+// are computed.  Returns the bytes the plan needs.
+size_t static_carve(mlp_pipe* h, unsigned char* base, size_t* zero_bytes) {
+    size_t off = 0;
+    auto take = [&](size_t bytes) {
+        unsigned char* p = base ? base + off : nullptr;
+        off = static_align_up(off + bytes);
+        return p;
+    };
+    size_t words = 0;   // (same counter layout as a handle's: one 128-byte line for the ticket, then per-128-row-block counters)
+    for (int l = 0; l < h->L; ++l) words += 32 + 2 * static_cast<size_t>(round_up(2 * ceil_div(h->widths[l + 1], 2 * kTileN) * h->m_blks, 32));
+    h->counters_words = words;
+    h->counters = reinterpret_cast<uint32_t*>(take(words * sizeof(uint32_t)));
+    if (base) {
+        uint32_t* p = h->counters;
+        for (int l = 0; l < h->L; ++l) {
+            const int t128 = round_up(2 * ceil_div(h->widths[l + 1], 2 * kTileN) * h->m_blks, 32);
+            h->ticket[l] = p;
+            p += 32;
+            h->arrive[l] = p;
+            p += t128;
+            h->ready[l] = p;
+            p += t128;
+        }
+    }
+    h->epoch = reinterpret_cast<unsigned long long*>(take(kMaxLayers * sizeof(unsigned long long)));
+    h->status = reinterpret_cast<uint32_t*>(take(sizeof(uint32_t)));
+    h->stats = reinterpret_cast<CtaStats*>(take(sizeof(CtaStats) * h->grid));
+    *zero_bytes = off;
+    for (int l = 0; l < h->L; ++l) h->d_table[l] = reinterpret_cast<UnitDesc*>(take(h->table[l].size() * sizeof(UnitDesc)));
+    for (int l = 0; l < h->L - 1; ++l) h->H[l] = reinterpret_cast<__nv_bfloat16*>(take(static_cast<size_t>(h->M) * h->widths[l + 1] * 2));
+    for (int l = 0; l < h->L; ++l) {
+        const size_t ws_bytes = h->split[l] > 1 ? static_cast<size_t>(h->tiles[l]) * h->split[l] * h->n_sub * h->tile_m * kTileN * sizeof(float) : 0;
+        h->ws[l] = ws_bytes ? reinterpret_cast<float*>(take(ws_bytes)) : nullptr;
+    }
+    return off;
+}
+
+bool static_same_problem(const mlp_pipe* h, int M, int L, const int* widths, int act) {
+    if (!h || h->M != M || h->L != L || h->act != act) return false;
+    for (int l = 0; l <= L; ++l)
+        if (h->widths[l] != widths[l]) return false;
+    return true;
+}
+
+// Plan (M, widths, act) as a default CTA_PIPELINED handle would, and point the plan at the array.  Host work only.
+int static_make_plan(StaticSlot& S, int M, int L, const int* widths, int act) {
+    mlp_mode m{};
+    m.kind = MLP_CTA_PIPELINED;
+    for (int l = 0; l < L; ++l)
+        if (static_cast<long long>(ceil_div(M, 256)) * ceil_div(widths[l + 1], 2 * kTileN) > 65535 || ceil_div(widths[l], kTileK) > 65535)
+            return fail(nullptr, MLP_ERR_UNSUPPORTED, "layer %d exceeds the unit table's 16-bit tile / K-block fields", l);
+    mlp_pipe* h = new (std::nothrow) mlp_pipe();
+    if (!h) return fail(nullptr, MLP_ERR_OOM, "host allocation failed");
+    h->M = M;
+    h->L = L;
+    for (int l = 0; l <= L; ++l) h->widths[l] = widths[l];
+    h->act = act;
+    h->mode = m;
+    cudaGetDevice(&h->dev);
+    h->num_sms = S.num_sms;
+    resolve(h);
+    for (int l = 0; l < L; ++l)
+        if (static_cast<long long>(ceil_div(widths[l + 1], kTileN)) * h->m_blks > 65535) {
+            delete h;
+            return fail(nullptr, MLP_ERR_UNSUPPORTED, "layer %d exceeds the unit table's 16-bit tile field", l);
+        }
+    size_t zero_bytes = 0;
+    const size_t need = static_carve(h, nullptr, &zero_bytes);
+    if (need > static_cast<size_t>(MLP_STATIC_SCRATCH_BYTES)) {
+        delete h;
+        return fail(nullptr, MLP_ERR_UNSUPPORTED,
+                    "mlp_pipe_run_static: this problem needs %zu bytes of scratch, the library's fixed array holds %zu "
+                    "(MLP_STATIC_SCRATCH_BYTES); use mlp_pipe_create / mlp_pipe_run for it",
+                    need, static_cast<size_t>(MLP_STATIC_SCRATCH_BYTES));
+    }
+    static_carve(h, S.base, &zero_bytes);
+    h->status_host = nullptr;      // no pinned mirror (that would be an allocation): a watchdog expiry stays on the device
+    h->status_host_dev = nullptr;
+    const int rc = build_base_params(h);   // encodes the tensor maps of the hidden activations (host only)
+    if (rc) {
+        g_create_error = h->last_error;
+        delete h;
+        return rc;
+    }
+    delete S.plan;   // (a plain host object: nothing in it was cudaMalloc'ed)
+    S.plan = h;
+    S.zero_bytes = zero_bytes;
+    return MLP_OK;
+}
+
+}  // namespace
+
+extern "C" int mlp_pipe_run_static(int M, int n_layers, const int* widths, int act, const void* X, const void* const* W, void* Y,
+                                   void* cuda_stream) {
+    const int L = n_layers;
+    if (!widths || L < 1 || L > kMaxLayers || M < 1) return fail(nullptr, MLP_ERR_INVALID, "bad M / n_layers / widths");
+    if (act < MLP_ACT_NONE || act > MLP_ACT_GELU_TANH) return fail(nullptr, MLP_ERR_INVALID, "bad act %d", act);
+    for (int l = 0; l <= L; ++l)
+        if (widths[l] < 8 || widths[l] % 8 != 0)
+            return fail(nullptr, MLP_ERR_INVALID, "width[%d] = %d must be a positive multiple of 8", l, widths[l]);
+    if (!W) return fail(nullptr, MLP_ERR_INVALID, "W is NULL");
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticSlot* S = nullptr;
+    int rc = static_slot_for_current_device(&S);
+    if (rc) return rc;
+    if (!static_same_problem(S->plan, M, L, widths, act) && (rc = static_make_plan(*S, M, L, widths, act))) return rc;
+    mlp_pipe* h = S->plan;
+    h->last_error.clear();
+    auto report = [&](int code) {   // errors of this handle-less call are read with mlp_pipe_last_error(NULL)
+        g_create_error = h->last_error;
+        return code;
+    };
+    if ((rc = check_ptr(h, X, "X")) || (rc = check_ptr(h, Y, "Y"))) return report(rc);
+    for (int l = 0; l < L; ++l)
+        if ((rc = check_ptr(h, W[l], "W[l]"))) return report(rc);
+
+    // The array still holds what the previous call (of any shape) left there.  What the protocol reads before it writes --
+    // tickets, arrival and ready counters, the epoch, the status word, the per-CTA records -- is cleared on the caller's
+    // stream; hidden activations and partials are always written before they are read, and the unit tables are re-sent.
+    cudaError_t e = cudaMemsetAsync(S->base, 0, S->zero_bytes, s);
+    for (int l = 0; l < L && e == cudaSuccess; ++l)
+        e = cudaMemcpyAsync(h->d_table[l], h->table[l].data(), h->table[l].size() * sizeof(UnitDesc), cudaMemcpyHostToDevice, s);
+    // (the attribute is per kernel, not per plan: raise it to the hardware limit so that no handle's launch is cut short)
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(mlp_pipe_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(nullptr, MLP_ERR_CUDA, "mlp_pipe_run_static set-up: %s", cudaGetErrorString(e));
+    }
+    KernelParams P = h->base;
+    if ((rc = lookup_tmap(h, h->cache_x, &h->cache_x_next, X, M, widths[0], h->tile_m, &P.tm_a[0]))) return report(rc);
+    for (int l = 0; l < L; ++l)
+        if ((rc = lookup_tmap(h, h->cache_w[l], &h->cache_w_next[l], W[l], widths[l + 1], widths[l], kTileN * h->n_sub, &P.tm_w[l])))
+            return report(rc);
+    P.layer[L - 1].out = static_cast<__nv_bfloat16*>(Y);
+    P.layer_begin = 0;   // one persistent (cooperative) launch over all layers, exactly as mlp_pipe_run's CTA_PIPELINED branch
+    P.layer_end = L;
+    P.m_off = 0;
+    P.m_end = M;
+    P.wait_flags = 1;
+    P.producer_ctas = h->producer_ctas;
+    P.epoch_counter = h->epoch;
+    P.stats = h->stats;
+    if ((rc = launch(h, P, s))) return report(rc);
+    return MLP_OK;
+}
