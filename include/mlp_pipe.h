@@ -133,7 +133,9 @@ enum {
                                        second stream over the remaining SMs, gated by cuStreamWaitValue32 on the first ready
                                        counter reaching this run's value; inside the consumer kernel every unit polls its ready
                                        counters as usual.  Not capturable into a CUDA graph (the wait value is per run), not
-                                       with MLP_FLAG_WORKQUEUE / PAIR / AUTOTUNE (UNSUPPORTED).                                 */
+                                       with MLP_FLAG_WORKQUEUE / PAIR / AUTOTUNE, not on a grid of 1 CTA -- each kernel needs
+                                       one of its own -- and not for chains other than 2 layers (UNSUPPORTED, from create and
+                                       from mlp_pipe_plan alike).                                                              */
 #define MLP_FLAG_AUTOTUNE 0x400u    /* measured plan search: the FIRST mlp_pipe_run on the handle (outside stream
                                        capture) tries the planner's candidate K-splits / ticket orders (and, unless tile_n is given,
                                        both unit heights 128 / 256) on the

@@ -655,8 +655,10 @@ void resolve(mlp_pipe* h) {
     }
     if (h->two_kernel) {   // producer kernel on s x grid CTAs, consumer kernel on the rest (sm_split; 0 or 1 is read as 1/2)
         const float sp2 = (m.sm_split <= 0.0f || m.sm_split >= 1.0f) ? 0.5f : m.sm_split;
-        h->lgrid[0] = h->lworkers[0] = std::min(h->grid - 1, std::max(1, static_cast<int>(h->grid * sp2 + 0.5f)));
-        h->lgrid[1] = h->lworkers[1] = h->grid - h->lgrid[0];
+        // (a grid of 1 cannot be partitioned: create and plan refuse it, two_kernel_problem(); the clamps only keep
+        // everything computed from the per-kernel grids well defined until they do)
+        h->lgrid[0] = h->lworkers[0] = std::max(1, std::min(h->grid - 1, std::max(1, static_cast<int>(h->grid * sp2 + 0.5f))));
+        h->lgrid[1] = h->lworkers[1] = std::max(1, h->grid - h->lgrid[0]);
     }
     const float s = (m.sm_split <= 0.0f) ? 1.0f : m.sm_split;
     h->producer_ctas = h->workers;  // (counted in workers)
@@ -763,6 +765,15 @@ void resolve(mlp_pipe* h) {
             fprintf(stderr, "%s\n", pl.pipelined ? "" : (std::string("  model ") + std::to_string(pl.makespan(l, l + 1))).c_str());
         }
     }
+}
+
+// What only the RESOLVED configuration can tell about MLP_FLAG_TWO_KERNEL: it is defined for 2 layers, and each of the two
+// kernels needs at least one CTA of its own.  NULL = fine.
+const char* two_kernel_problem(const mlp_pipe& h) {
+    if (!(h.mode.flags & MLP_FLAG_TWO_KERNEL)) return nullptr;
+    if (h.L != 2) return "MLP_FLAG_TWO_KERNEL needs a 2-layer handle";
+    if (h.grid < 2) return "MLP_FLAG_TWO_KERNEL needs at least 2 CTAs, one for each kernel (resolved grid = 1)";
+    return nullptr;
 }
 
 int build_base_params(mlp_pipe* h) {
@@ -1037,6 +1048,10 @@ int create_impl(mlp_pipe** out, int M, int L, const int* widths, int dtype, int 
     h->dev = dev;
     h->num_sms = prop.multiProcessorCount;
     resolve(h);
+    if (const char* why = two_kernel_problem(*h)) {
+        delete h;
+        return fail(nullptr, MLP_ERR_UNSUPPORTED, "%s", why);
+    }
     for (int l = 0; l < L; ++l) {  // the unit table stores tile ids and K-block bounds in 16 bits, the K-slice index in 8
         const long long tiles128 = static_cast<long long>(ceil_div(widths[l + 1], kTileN)) * h->m_blks;
         if (tiles128 > 65535 || ceil_div(widths[l], kTileK) > 65535) {
@@ -1666,7 +1681,7 @@ int mlp_pipe_plan(int M, int n_layers, const int* widths, const mlp_mode* mode, 
         if (static_cast<long long>(ceil_div(M, 256)) * ceil_div(widths[l + 1], 2 * kTileN) > 65535 || ceil_div(widths[l], kTileK) > 65535)
             return MLP_ERR_UNSUPPORTED;
     resolve(&h);
-    if (!fits_unit_table(h)) return MLP_ERR_UNSUPPORTED;
+    if (!fits_unit_table(h) || two_kernel_problem(h)) return MLP_ERR_UNSUPPORTED;
     memset(out, 0, sizeof *out);
     out->tile_m = h.tile_m;
     out->tile_n = kTileN * (h.pair ? 2 : h.n_sub);
@@ -1710,7 +1725,7 @@ int mlp_pipe_plan_units(int M, int n_layers, const int* widths, const mlp_mode* 
         if (static_cast<long long>(ceil_div(M, 256)) * ceil_div(widths[l + 1], 2 * kTileN) > 65535 || ceil_div(widths[l], kTileK) > 65535)
             return MLP_ERR_UNSUPPORTED;
     resolve(&h);
-    if (!fits_unit_table(h)) return MLP_ERR_UNSUPPORTED;
+    if (!fits_unit_table(h) || two_kernel_problem(h)) return MLP_ERR_UNSUPPORTED;
     const std::vector<UnitDesc>& t = h.table[layer];
     const int n = std::min<int>(max_units, static_cast<int>(t.size()));
     for (int i = 0; i < n; ++i) {

@@ -137,6 +137,27 @@ def test_coresident_and_two_kernel_grids():
     assert B.load().mlp_pipe_plan(128, 4, w4, ctypes.byref(bad), 148, ctypes.byref(out)) == B.MLP_ERR_INVALID
 
 
+def test_two_kernel_needs_a_cta_for_each_kernel():
+    """A grid of one CTA cannot be split into a producer and a consumer kernel: plan and plan_units refuse it (create runs
+    the same check) instead of planning a producer launch of 0 CTAs; a grid of 2 is the smallest that works (1 + 1).  A chain
+    that is not 2 layers long is refused by the planner as it is by create."""
+    import ctypes
+    lib = B.load()
+    cfg = inputs.CONFIGS[0]
+    w = (ctypes.c_int * 3)(*cfg.widths)
+    out, units, n = B.mlp_plan(), (B.mlp_unit * 8)(), ctypes.c_int()
+    for sms, grid in ((148, 1), (1, 0)):
+        m = B.make_mode(P, flags=B.MLP_FLAG_TWO_KERNEL, grid=grid)
+        assert lib.mlp_pipe_plan(cfg.M, 2, w, ctypes.byref(m), sms, ctypes.byref(out)) == B.MLP_ERR_UNSUPPORTED
+        assert lib.mlp_pipe_plan_units(cfg.M, 2, w, ctypes.byref(m), sms, 0, units, 8, ctypes.byref(n)) == B.MLP_ERR_UNSUPPORTED
+    ok, tables = B.plan(cfg.M, cfg.widths, B.make_mode(P, flags=B.MLP_FLAG_TWO_KERNEL, grid=2), num_sms=148)
+    assert ok.grid == 2
+    _check_tables(cfg.M, cfg.widths, ok, tables)
+    w4 = (ctypes.c_int * 5)(*inputs.CONFIGS[4].widths)
+    m = B.make_mode(P, flags=B.MLP_FLAG_TWO_KERNEL)
+    assert lib.mlp_pipe_plan(128, 4, w4, ctypes.byref(m), 148, ctypes.byref(out)) == B.MLP_ERR_UNSUPPORTED
+
+
 def test_plan_rejects_bad_arguments():
     import ctypes
     lib = B.load()
