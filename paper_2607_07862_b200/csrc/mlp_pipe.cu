@@ -106,7 +106,7 @@ struct mlp_pipe {
     cudaEvent_t ev_fork = nullptr;
     cudaEvent_t ev_t0 = nullptr, ev_t1 = nullptr;  // autotune of MICROBATCH: fork .. join time
     std::vector<cudaEvent_t> ev_done;  // [L][chunks]
-    bool poisoned_state = false;       // a watchdog expiry was seen: counters must be reset
+    bool poisoned_state = false;       // a watchdog expiry was seen, or a two-kernel run was only half enqueued: counters must be reset
     unsigned long long tk_epoch = 0;   // MLP_FLAG_TWO_KERNEL: runs since the last reset (= the device epoch when this run starts)
     bool drop_fired = false;           // MLP_FLAG_DEBUG_DROP_PUBLISH is one-shot: only the handle's first run drops its publish
     unsigned long long runs = 0;
@@ -1192,8 +1192,20 @@ int run_core(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStre
         if (cudaStreamIsCapturing(s, &cap) == cudaSuccess && cap != cudaStreamCaptureStatusNone)
             return fail(h, MLP_ERR_UNSUPPORTED, "MLP_FLAG_TWO_KERNEL cannot be captured (the wait value is computed per run on the host)");
         CUDA_TRY(h, cudaEventRecord(h->ev_fork, s));
+        // Once the producer kernel is enqueued, an error must not leave the internal streams detached from the caller's,
+        // nor the host's run count behind the device's: rejoin, and have the next run reset the protocol state.
+        bool producer_enqueued = false;
+        auto bail = [&](int code) {
+            if (producer_enqueued) {
+                for (int j = 0; j < 2; ++j)
+                    if (cudaEventRecord(h->tk_done[j], h->tk_stream[j]) == cudaSuccess) cudaStreamWaitEvent(s, h->tk_done[j], 0);
+                cudaGetLastError();
+                h->poisoned_state = true;
+            }
+            return code;
+        };
         for (int l = 0; l < 2; ++l) {
-            CUDA_TRY(h, cudaStreamWaitEvent(h->tk_stream[l], h->ev_fork, 0));
+            if (cudaStreamWaitEvent(h->tk_stream[l], h->ev_fork, 0) != cudaSuccess) return bail(fail(h, MLP_ERR_CUDA, "cudaStreamWaitEvent failed"));
             P.layer_begin = l;
             P.layer_end = l + 1;
             P.m_off = 0;
@@ -1204,16 +1216,29 @@ int run_core(mlp_pipe* h, const void* X, const void* const* W, void* Y, cudaStre
             P.epoch_counter = h->epoch + l;
             P.stats = h->stats + static_cast<size_t>(l) * h->grid;
             if (l > 0) {
-                const uint32_t target = static_cast<uint32_t>((h->tk_epoch + 1ull) * static_cast<unsigned long long>(h->ready_inc[0]));
-                const uint32_t* first = h->ready[0] + h->table[0][0].tile;   // the tile of ticket 0 turns first
-                const CUresult r = h->wait_value32(reinterpret_cast<CUstream>(h->tk_stream[l]), reinterpret_cast<CUdeviceptr>(first), target,
-                                                   CU_STREAM_WAIT_VALUE_GEQ);
-                if (r != CUDA_SUCCESS) return fail(h, MLP_ERR_CUDA, "cuStreamWaitValue32 failed (%d)", static_cast<int>(r));
+                // The gate sits OUTSIDE the kernels' flag watchdog (timeout_ms), so it must watch a counter that is certain to
+                // turn: the tile of the first ticket (it turns first; without CTA pairs a unit's counter index is its tile id,
+                // kernel.cuh `ctile`).  A producer always publishes, even after its own watchdog let it go -- except the one
+                // tile that MLP_FLAG_DEBUG_DROP_PUBLISH silences on purpose: then the gate watches the first ticket of another
+                // tile, and no gate at all if there is none (the consumer kernel starts at once and its units starve inside
+                // the kernel, where the watchdog sees them).
+                const bool drop = (P.flags & MLP_FLAG_DEBUG_DROP_PUBLISH) != 0;
+                int gate = -1;
+                for (size_t t = 0; t < h->table[0].size() && gate < 0; ++t)
+                    if (h->table[0][t].kind == kUnitMma && !(drop && h->table[0][t].tile == 0)) gate = h->table[0][t].tile;
+                if (gate >= 0) {
+                    const uint32_t target = static_cast<uint32_t>((h->tk_epoch + 1ull) * static_cast<unsigned long long>(h->ready_inc[0]));
+                    const CUresult r = h->wait_value32(reinterpret_cast<CUstream>(h->tk_stream[l]), reinterpret_cast<CUdeviceptr>(h->ready[0] + gate),
+                                                       target, CU_STREAM_WAIT_VALUE_GEQ);
+                    if (r != CUDA_SUCCESS) return bail(fail(h, MLP_ERR_CUDA, "cuStreamWaitValue32 failed (%d)", static_cast<int>(r)));
+                }
             }
-            if ((rc = launch(h, P, h->tk_stream[l]))) return rc;
-            CUDA_TRY(h, cudaEventRecord(h->tk_done[l], h->tk_stream[l]));
+            if ((rc = launch(h, P, h->tk_stream[l]))) return bail(rc);
+            if (l == 0) producer_enqueued = true;
+            if (cudaEventRecord(h->tk_done[l], h->tk_stream[l]) != cudaSuccess) return bail(fail(h, MLP_ERR_CUDA, "cudaEventRecord failed"));
         }
-        for (int l = 0; l < 2; ++l) CUDA_TRY(h, cudaStreamWaitEvent(s, h->tk_done[l], 0));
+        for (int l = 0; l < 2; ++l)
+            if (cudaStreamWaitEvent(s, h->tk_done[l], 0) != cudaSuccess) return bail(fail(h, MLP_ERR_CUDA, "cudaStreamWaitEvent failed"));
         h->tk_epoch++;
     } else if (kind == MLP_CTA_PIPELINED) {
         // one persistent launch; tickets order all units of layer l before those of layer l+1

@@ -246,12 +246,14 @@ def test_run_host_matches_device_path():
     p.close()
 
 
-@pytest.mark.parametrize("extra", [0, B.MLP_FLAG_WORKQUEUE, B.MLP_FLAG_PAIR])
+@pytest.mark.parametrize("extra", [0, B.MLP_FLAG_WORKQUEUE, B.MLP_FLAG_PAIR, B.MLP_FLAG_TWO_KERNEL])
 def test_watchdog_turns_a_hang_into_timeout(extra):
     """MLP_FLAG_DEBUG_DROP_PUBLISH: the producer of tile 0 never publishes on the handle's FIRST run, so the consumers of
     that tile starve.  The flag-poll watchdog must end the kernel (no hang), MLP_ERR_TIMEOUT must be reported -- by
     mlp_pipe_stats, and by the next mlp_pipe_run WITHOUT any stats call (the kernel mirrors its status word into pinned
-    host memory) --, the handle must be reset, and the runs after that must be bit-exact again."""
+    host memory) --, the handle must be reset, and the runs after that must be bit-exact again.
+    With MLP_FLAG_TWO_KERNEL the consumer KERNEL is gated by a stream wait that no watchdog covers: the gate must then
+    watch a tile that is published, so that the starvation happens inside the kernel, where it is bounded."""
     cfg = inputs.get_config(0, "exact")
     X, Ws, outs, _ = oracle_outs(cfg)
     Xd, Wd = X.cuda(), [w.cuda() for w in Ws]
