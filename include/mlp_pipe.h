@@ -118,8 +118,11 @@ enum {
                                        the deterministic way to exercise MLP_ERR_TIMEOUT.  One-shot: only the FIRST run of the
                                        handle drops the publish, so the runs after the reset are clean                            */
 #define MLP_FLAG_NO_COOPERATIVE 0x8000u /* launch WITHOUT cudaLaunchAttributeCooperative.  By default every launch in which a CTA
-                                       may wait on another CTA (CTA_PIPELINED; split-K reduce units in any mode) is cooperative:
-                                       the grid starts only when all its CTAs fit on the device at once.  With this flag the
+                                       may wait on another CTA (CTA_PIPELINED, also as the two kernels of MLP_FLAG_TWO_KERNEL;
+                                       split-K reduce units in any mode, also in the sibling launches of MLP_FLAG_MB_CORESIDENT)
+                                       is cooperative: the grid starts only when all its CTAs fit on the device at once.  The one
+                                       exception is MLP_FLAG_PDL, whose dependent launches are meant to start while the launch
+                                       before still holds SMs (measured: cooperative costs the sibling modes nothing).  With this flag the
                                        caller guarantees that (an otherwise idle GPU, no second handle running concurrently);
                                        otherwise waiting CTAs can starve CTAs that are not yet resident until the watchdog.   */
 #define MLP_FLAG_MB_CORESIDENT 0x10000u /* MICROBATCH only: every launch gets num_SMs / min(L, chunks) CTAs instead of one per SM, so

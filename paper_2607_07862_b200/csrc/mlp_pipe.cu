@@ -907,9 +907,11 @@ int launch(mlp_pipe* h, KernelParams& P, cudaStream_t s) {
     // (behind another kernel, or a second handle on another stream, it queues instead of deadlocking until the watchdog).
     bool waits = P.wait_flags != 0;
     for (int l = P.layer_begin; l < P.layer_end; ++l) waits = waits || P.layer[l].reduce_mode == kReduceUnits;
-    // (not for launches that are MEANT to share the device with a sibling launch of the same handle: the two-kernel
-    // pipeline and co-resident micro-batches size their grids so that the siblings fit together)
-    if (waits && !(h->mode.flags & (MLP_FLAG_NO_COOPERATIVE | MLP_FLAG_PDL | MLP_FLAG_TWO_KERNEL | MLP_FLAG_MB_CORESIDENT))) {
+    // (The sibling launches of one handle -- the two kernels of MLP_FLAG_TWO_KERNEL, the per-stream launches of
+    // MLP_FLAG_MB_CORESIDENT -- are cooperative too: a cooperative launch only needs its OWN grid to fit, and these grids are
+    // sized so that the siblings fit side by side.  Only a programmatic dependent launch cannot be cooperative: it is meant to
+    // start while its predecessor still holds SMs.)
+    if (waits && !(h->mode.flags & (MLP_FLAG_NO_COOPERATIVE | MLP_FLAG_PDL))) {
         attr[cfg.numAttrs].id = cudaLaunchAttributeCooperative;
         attr[cfg.numAttrs].val.cooperative = 1;
         cfg.attrs = attr;

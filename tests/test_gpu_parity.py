@@ -314,6 +314,32 @@ def test_two_pipelined_handles_on_two_streams():
 TK = B.MLP_FLAG_TWO_KERNEL
 
 
+@pytest.mark.parametrize("kw", [dict(kind=P, flags=B.MLP_FLAG_TWO_KERNEL, split_k=4),
+                                dict(kind=MB, chunks=2, flags=B.MLP_FLAG_MB_CORESIDENT, split_k=4)], ids=["two_kernel", "mb_coresident"])
+def test_two_handles_on_two_streams_sibling_launch_modes(kw):
+    """The same co-residency guarantee for the modes whose handle issues SIBLING launches that share the device (the two
+    kernels of MLP_FLAG_TWO_KERNEL, the per-stream launches of MLP_FLAG_MB_CORESIDENT): their launches are cooperative as
+    well, so two such handles fed from two streams at once queue behind each other instead of starving half-resident
+    grids until the watchdog.  split_k = 4 gives every layer reduce units, i.e. CTAs that wait in every launch."""
+    cfg = inputs.Config("two_handles", 64, (1024, 4096, 1024), B.MLP_ACT_RELU, "exact", 5)
+    X, Ws, outs, _ = oracle_outs(cfg)
+    Xd, Wd = X.cuda(), [w.cuda() for w in Ws]
+    ps = [B.MlpPipe(cfg.M, cfg.widths, cfg.act, B.make_mode(timeout_ms=500, **kw)) for _ in range(2)]
+    streams = [torch.cuda.Stream() for _ in range(2)]
+    Ys = [torch.zeros((cfg.M, cfg.widths[-1]), dtype=torch.bfloat16, device="cuda") for _ in range(2)]
+    torch.cuda.synchronize()
+    for i in range(100):
+        for k in range(2):
+            with torch.cuda.stream(streams[k]):
+                ps[k].run(Xd, Wd, Ys[k], stream=streams[k])
+    torch.cuda.synchronize()
+    for k in range(2):
+        st = ps[k].stats()
+        assert st.status == 0 and st.ready_ok == 1
+        assert np.array_equal(inputs.as_u16(Ys[k].cpu()), outs[-1])
+        ps[k].close()
+
+
 @pytest.mark.parametrize("kw", [dict(), dict(sm_split=0.25, split_k=4), dict(sm_split=0.75, split_k=2), dict(split_k_layer=[2, 8]),
                                 dict(flags=B.MLP_FLAG_DEBUG_DELAY, split_k=4), dict(flags=B.MLP_FLAG_DEBUG_DELAY | B.MLP_FLAG_DEBUG_REVERSE),
                                 dict(flags=B.MLP_FLAG_ACQUIRE_LOADS, split_k=4)], ids=[str(i) for i in range(7)])
