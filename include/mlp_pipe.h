@@ -238,7 +238,7 @@ typedef struct {
     uint64_t runs;                                /* completed launches counted by the device epoch   */
     uint64_t flag_stall_cycles_sum;               /* sum over CTAs of SM cycles spent polling flags    */
     uint64_t flag_stall_cycles_max;               /* max over CTAs                                    */
-    uint64_t flag_polls;                          /* ld.acquire polls that found the slice not ready  */
+    uint64_t flag_polls;                          /* polls (relaxed, or ld.acquire with MLP_FLAG_ACQUIRE_LOADS) that found the slice not ready */
     uint64_t kernel_cycles_max;                   /* max over CTAs of the CTA's lifetime in SM cycles */
     uint32_t units_done[MLP_MAX_LAYERS];          /* units executed per layer, summed over CTAs       */
     uint32_t units_by_consumer_ctas[MLP_MAX_LAYERS]; /* of which by CTAs in the consumer-first group  */
@@ -253,8 +253,9 @@ int mlp_pipe_stats(mlp_pipe* h, mlp_stats* out, size_t bytes);
 /*
  * Profiling hook (the paper's in-kernel timestamp instrumentation): per-CTA records
  * of the most recent launch of launch class `cls` (0 for CTA_PIPELINED; the layer index for
- * SEQUENTIAL / MICROBATCH).  Copies min(max_records, grid) records to the host array `out` and
- * returns the number copied through *n_out.  Synchronises the device.
+ * SEQUENTIAL / MICROBATCH / the two kernels of MLP_FLAG_TWO_KERNEL).  Copies min(max_records, CTAs of that class's
+ * launch) records to the host array `out` -- the grid, except under MLP_FLAG_TWO_KERNEL, where each kernel has its own
+ * share of it -- and returns the number copied through *n_out.  Synchronises the device.
  */
 #define MLP_UNIT_TRACE 12
 typedef struct {

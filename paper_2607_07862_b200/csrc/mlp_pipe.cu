@@ -1302,16 +1302,19 @@ int last_span_us(mlp_pipe* h, double* out) {
     const int classes = launch_classes(h);
     std::vector<CtaStats> cs(static_cast<size_t>(classes) * h->grid);
     CUDA_TRY(h, cudaMemcpy(cs.data(), h->stats, cs.size() * sizeof(CtaStats), cudaMemcpyDeviceToHost));
+    // (the two kernels of MLP_FLAG_TWO_KERNEL overlap by design: their span is first start .. last exit over BOTH classes)
     double total = 0.0;
+    unsigned long long t0 = ~0ull, t1 = 0;
     for (int c = 0; c < classes; ++c) {
-        unsigned long long t0 = ~0ull, t1 = 0;
+        if (!h->two_kernel) t0 = ~0ull, t1 = 0;
         for (int b = 0; b < h->lgrid[classes == 1 ? 0 : c]; ++b) {
             const CtaStats& st = cs[static_cast<size_t>(c) * h->grid + b];
             t0 = std::min(t0, st.ts[0]);
             t1 = std::max(t1, st.ts[7]);
         }
-        total += (t1 - t0) * 1e-3;
+        if (!h->two_kernel) total += (t1 - t0) * 1e-3;
     }
+    if (h->two_kernel) total = (t1 - t0) * 1e-3;
     *out = total;
     return MLP_OK;
 }
@@ -1645,7 +1648,7 @@ int mlp_pipe_cta_records(mlp_pipe* h, int cls, mlp_cta_record* out, int max_reco
     const int classes = launch_classes(h);
     if (cls < 0 || cls >= classes) return fail(h, MLP_ERR_INVALID, "bad launch class %d", cls);
     CUDA_TRY(h, cudaDeviceSynchronize());
-    const int n = std::min(max_records, h->grid);
+    const int n = std::min(max_records, h->lgrid[classes == 1 ? 0 : cls]);   // the CTAs that class really ran (two-kernel: its own grid)
     CUDA_TRY(h, cudaMemcpy(out, h->stats + static_cast<size_t>(cls) * h->grid, sizeof(CtaStats) * n, cudaMemcpyDeviceToHost));
     *n_out = n;
     return MLP_OK;

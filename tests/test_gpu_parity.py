@@ -361,6 +361,10 @@ def test_two_kernel_stream_wait_pipeline(kw):
     assert st.ready_ok == 1 and st.status == 0 and st.runs == 30
     assert st.units_done[0] == st.units[0] and st.units_done[1] == st.units[1]
     assert 0 < st.producer_ctas < st.grid
+    # per-CTA records follow the per-kernel grids: class 0 = the producer kernel's CTAs, class 1 = the consumer kernel's
+    rec = [p.cta_records(c, 256) for c in range(2)]
+    assert len(rec[0]) == st.producer_ctas and len(rec[1]) == st.grid - st.producer_ctas
+    assert all(r.ts[7] > r.ts[0] > 0 for c in range(2) for r in rec[c]), "every returned record belongs to a CTA that ran"
     p.close()
 
 
