@@ -30,30 +30,33 @@ def main() -> int:
     ap.add_argument("--split-k", type=str, default="")
     ap.add_argument("--tile-n", type=int, default=0)
     ap.add_argument("--act", type=int, default=-1, help="override the activation: 0 none, 1 ReLU, 2 GeLU-tanh")
-    ap.add_argument("--sm-mhz", type=float, default=1965.0)
+    ap.add_argument("--sm-mhz", type=float, default=0.0,
+                    help="SM clock for cycles -> us; 0 = the median clock sampled (NVML) while the timed runs executed")
     args = ap.parse_args()
 
     import torch
 
-    import bench
     from paper_2607_07862_b200 import binding as B
-    from paper_2607_07862_b200 import inputs
+    from paper_2607_07862_b200 import inputs, timing
 
     cfg = inputs.CONFIGS[args.config]
     if args.act >= 0:
         cfg = inputs.Config(cfg.name + f"_act{args.act}", cfg.M, cfg.widths, args.act, cfg.dist, cfg.seed)
     kind = B.MLP_CTA_PIPELINED if args.mode == "pipelined" else B.MLP_SEQUENTIAL
     flags = (0 if args.no_autotune else B.MLP_FLAG_AUTOTUNE) | (B.MLP_FLAG_WORKQUEUE if args.workqueue else 0) | (B.MLP_FLAG_PAIR if args.pair else 0)
-    X, sets = bench.device_inputs(torch, cfg, bench.weight_sets_for(cfg))
+    X, sets = timing.device_inputs(torch, cfg, timing.weight_sets_for(cfg))
     Y = torch.empty((cfg.M, cfg.widths[-1]), dtype=torch.bfloat16, device="cuda")
     split = [int(x) for x in args.split_k.split(",")] if args.split_k else []
     p = B.MlpPipe(cfg.M, cfg.widths, cfg.act, B.make_mode(kind, flags=flags, split_k_layer=split, tile_n=args.tile_n))
-    lat, _ = bench.time_steps(torch, p, X, sets, Y, 50, 10)
+    sampler = timing.ClockSampler(timing.nvml_index_for(torch, torch.cuda.current_device()))
+    lat, clocks = timing.time_steps(torch, p, X, sets, Y, 50, 10, sampler)
     st = p.stats()
     L = cfg.n_layers
     print(f"{cfg.name}: CUDA-event median {lat['median']:.1f} us; unit tile {st.tile_n}x{st.tile_m}, stages {st.stages}, "
           f"K-split {list(st.split_k)[:L]}, reduce mode {list(st.reduce_mode)[:L]}, tickets {list(st.units)[:L]}")
-    cyc = args.sm_mhz  # SM cycles per us
+    # SM cycles per us: the clock the runs really had (an idle-to-busy GPU is not at its maximum clock), else the maximum
+    cyc = args.sm_mhz or (clocks or {}).get("sm_mhz") or (clocks or {}).get("sm_max_mhz") or 1965.0
+    print(f"SM clock for cycle counts: {cyc:.0f} MHz ({'given' if args.sm_mhz else 'sampled during the timed runs'})")
     for cls in range(1 if kind == B.MLP_CTA_PIPELINED else L):
         recs = p.cta_records(cls)
         t0 = min(r.ts[0] for r in recs)
