@@ -681,26 +681,82 @@ def test_many_m_blocks_rasterised_order(kw):
         assert st.units[0] >= 4 * 3
 
 
-@pytest.mark.parametrize("M", [1024, 4096])
-def test_paper_shape_sampled_rows(M):
-    """The paper's own workload shape (2 layers, no activation, 8192 x 8192 weights).  M = 4096 is
-    16 M-blocks = two rasterisation groups of 8 M-blocks (mlp_pipe.cu: build_table): token rows from EVERY 256-row M-block
-    (first, an inner and the last row of each) against the oracle, CTA_PIPELINED with and without CTA pairs and
-    SEQUENTIAL."""
-    cfg = inputs.Config(f"paper_{M}", M, (8192, 8192, 8192), B.MLP_ACT_NONE, "normal", 7)
+def _paper_case(M, rows, modes, seed=7):
+    """The paper's own workload shape (2 layers, no activation, 8192 x 8192 weights) at M tokens: H and Y of
+    the token rows `rows` (None = every row) against the oracle, in every mode of `modes`.  Token rows are independent, so the
+    oracle runs on exactly those rows of X."""
+    cfg = inputs.Config(f"paper_{M}", M, (8192, 8192, 8192), B.MLP_ACT_NONE, "normal", seed)
     X, Ws = inputs.make_inputs(cfg)
-    rows = sorted(set(r for b in range(0, M, 256) for r in (b, b + 97 + (b // 256) % 64, b + 255)))
-    outs, _ = oracle.mlp_chain(inputs.as_u16(X)[rows].copy(), [inputs.as_u16(w) for w in Ws], cfg.act)
-    for mode in (B.make_mode(P), B.make_mode(P, flags=PAIR), B.make_mode(S)):
+    Xu = inputs.as_u16(X)
+    outs, _ = oracle.mlp_chain(Xu if rows is None else Xu[rows].copy(), [inputs.as_u16(w) for w in Ws], cfg.act)
+    sel = slice(None) if rows is None else rows
+    for mode in modes:
         got, hs, st = run_gpu(cfg, mode, X, Ws)
         assert st.status == 0 and st.ready_ok == 1
+        for l in range(cfg.n_layers):
+            assert st.units_done[l] == st.units[l]
         if M >= 2048:
-            assert st.tile_m == 256 and M // st.tile_m >= 16   # >= 2 rasterisation groups
-        e = oracle.rel_err(hs[0][rows], outs[0])
+            assert st.tile_m == 256 and (M // (mode.chunks or 1)) // st.tile_m >= 16   # >= 2 rasterisation groups per launch
+        e = oracle.rel_err(hs[0][sel], outs[0])
         assert e["nan"] == 0 and e["err"] <= TOL, e
-        e = oracle.rel_err(got[rows], outs[-1])
+        e = oracle.rel_err(got[sel], outs[-1])
         assert e["nan"] == 0 and e["err"] <= TOL, e
         assert not np.isnan(oracle.u16_to_f64(got)).any()
+
+
+def test_paper_shape_sampled_rows_1024():
+    """M = 1024 (4 M-blocks): first, an inner and the last token row of every 256-row M-block, CTA_PIPELINED with and without
+    CTA pairs and SEQUENTIAL."""
+    M = 1024
+    rows = sorted(set(r for b in range(0, M, 256) for r in (b, b + 97 + (b // 256) % 64, b + 255)))
+    _paper_case(M, rows, (B.make_mode(P), B.make_mode(P, flags=PAIR), B.make_mode(S)))
+
+
+def test_paper_shape_every_element_4096():
+    """M = 4096 is 16 M-blocks = two rasterisation groups of 8 M-blocks (mlp_pipe.cu: build_table).  EVERY element of H and of
+    Y against the oracle (a token row is a TMEM column of the swap-AB tile: all 16 epilogue chunks of every 256-token tile
+    are compared), CTA_PIPELINED with and without CTA pairs and SEQUENTIAL."""
+    _paper_case(4096, None, (B.make_mode(P), B.make_mode(P, flags=PAIR), B.make_mode(S)))
+
+
+def test_paper_shape_16384():
+    """The shape the paper's headline numbers are quoted on: M = 16384 = 64 M-blocks = 8 rasterisation
+    groups.  Compared with the oracle: three token rows of EVERY 256-row M-block plus one M-block in full (256 consecutive
+    rows: every 16-column epilogue chunk of a tile_m = 256 tile), in CTA_PIPELINED, CTA_PIPELINED + CTA pairs, SEQUENTIAL +
+    CTA pairs and MICROBATCH(4)."""
+    M = 16384
+    rows = set(r for b in range(0, M, 256) for r in (b, b + 97 + (b // 256) % 64, b + 255))
+    rows |= set(range(37 * 256, 38 * 256))
+    _paper_case(M, sorted(rows), (B.make_mode(P), B.make_mode(P, flags=PAIR), B.make_mode(S, flags=PAIR), B.make_mode(MB, chunks=4)))
+
+
+def test_paper_scale_exact_mode_rasterised_order():
+    """Bit-exactness at the paper's scale: 8192 x 8192 weights, M = 2304 = 9 M-blocks (one full rasterisation group of 8 and a
+    ragged one), integer inputs in {-2..2}, no activation.  The certificate that makes the comparison order-insensitive is
+    analytic here (the oracle's own int64 check is run on a row sample only -- it is 20x slower than the oracle): all terms
+    are integers, and sum_k |a_k| |w_k| < 2^24 for every output element (float64 matmul of the absolute values, exact for
+    integers of this size), so every partial sum in ANY order is an integer below 2^24 and fp32 holds it exactly.  Whatever
+    order the rasterised tickets, the K-slices and the reduce units add in, H and Y must then equal the oracle's bits."""
+    cfg = inputs.Config("paper_exact", 2304, (8192, 8192, 8192), B.MLP_ACT_NONE, "exact", 11)
+    X, Ws = inputs.make_inputs(cfg)
+    Xu, Wu = inputs.as_u16(X), [inputs.as_u16(w) for w in Ws]
+    outs, _ = oracle.mlp_chain(Xu, Wu, cfg.act)
+    a = oracle.u16_to_f64(Xu)
+    for l, w in enumerate(Wu):
+        wf = oracle.u16_to_f64(w)
+        assert np.array_equal(a, np.rint(a)) and np.array_equal(wf, np.rint(wf))
+        bound = float((np.abs(a) @ np.abs(wf).T).max())
+        assert bound < 2 ** 24, (l, bound)
+        a = oracle.u16_to_f64(outs[l])
+    sample = list(range(0, cfg.M, 256))   # one token row per M-block through the oracle's int64 certificate as well
+    _, certs = oracle.mlp_chain(Xu[sample].copy(), Wu, cfg.act, want_cert=True)
+    for mx, bad, nonint in certs:
+        assert bad == 0 and nonint == 0 and mx < 2 ** 24
+    for mode in (B.make_mode(P), B.make_mode(P, flags=PAIR), B.make_mode(P, split_k=2), B.make_mode(S)):
+        got, hs, st = run_gpu(cfg, mode, X, Ws)
+        assert st.status == 0 and st.ready_ok == 1 and st.tile_m == 256
+        assert np.array_equal(hs[0], outs[0]), "H not bit-exact"
+        assert np.array_equal(got, outs[-1]), "Y not bit-exact"
 
 
 def test_bench_custom_shape_line_is_well_formed():
