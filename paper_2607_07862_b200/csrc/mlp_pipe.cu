@@ -34,6 +34,10 @@ struct TmapCacheEntry {
 };
 
 constexpr int kTmapCache = 8;
+// The dynamic shared-memory limit is an attribute of the kernel, shared by every handle of the process: it is always raised
+// to the hardware maximum (227 KB per CTA on sm_100), never set to one handle's own need -- a handle created later with
+// smaller rings would otherwise cut it below what an earlier, still live handle launches with.
+constexpr int kMaxDynamicSmem = 227 * 1024;
 
 }  // namespace
 
@@ -1080,8 +1084,8 @@ int create_impl(mlp_pipe** out, int M, int L, const int* widths, int dtype, int 
         }                                                                            \
     } while (0)
 
-    if (h->pair) CREATE_TRY(cudaFuncSetAttribute(mlp_pipe_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(h->smem_bytes)));
-    else CREATE_TRY(cudaFuncSetAttribute(mlp_pipe_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(h->smem_bytes)));
+    if (h->pair) CREATE_TRY(cudaFuncSetAttribute(mlp_pipe_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynamicSmem));
+    else CREATE_TRY(cudaFuncSetAttribute(mlp_pipe_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynamicSmem));
     for (int l = 0; l < L - 1; ++l) CREATE_TRY(cudaMalloc(&h->H[l], static_cast<size_t>(M) * widths[l + 1] * 2));
     // counters are laid out for 128-row tiles (the larger count), so that the measured search may switch tile_n
     size_t words = 0;
@@ -1324,8 +1328,8 @@ int last_span_us(mlp_pipe* h, double* out) {
 int reshape(mlp_pipe* h, int tile_n) {
     h->mode.tile_n = tile_n;
     resolve(h);
-    if (h->pair) CUDA_TRY(h, cudaFuncSetAttribute(mlp_pipe_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(h->smem_bytes)));
-    else CUDA_TRY(h, cudaFuncSetAttribute(mlp_pipe_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(h->smem_bytes)));
+    if (h->pair) CUDA_TRY(h, cudaFuncSetAttribute(mlp_pipe_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynamicSmem));
+    else CUDA_TRY(h, cudaFuncSetAttribute(mlp_pipe_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynamicSmem));
     for (int l = 0; l < kMaxLayers; ++l)
         for (int i = 0; i < kTmapCache; ++i) h->cache_w[l][i].ptr = nullptr;
     return MLP_OK;
@@ -1971,7 +1975,7 @@ extern "C" int mlp_pipe_run_static(int M, int n_layers, const int* widths, int a
     for (int l = 0; l < L && e == cudaSuccess; ++l)
         e = cudaMemcpyAsync(h->d_table[l], h->table[l].data(), h->table[l].size() * sizeof(UnitDesc), cudaMemcpyHostToDevice, s);
     // (the attribute is per kernel, not per plan: raise it to the hardware limit so that no handle's launch is cut short)
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(mlp_pipe_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(mlp_pipe_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynamicSmem);
     if (e != cudaSuccess) {
         cudaGetLastError();
         return fail(nullptr, MLP_ERR_CUDA, "mlp_pipe_run_static set-up: %s", cudaGetErrorString(e));

@@ -311,6 +311,26 @@ def test_two_pipelined_handles_on_two_streams():
         ps[k].close()
 
 
+def test_handles_with_different_shared_memory_needs_coexist():
+    """The dynamic shared-memory limit is an attribute of the KERNEL, not of a handle: a handle created later with smaller
+    rings (a decode-sized tile, 108 KB) must not cut the limit below what an earlier, still live handle launches with
+    (a 256-token tile, 210 KB) -- and the other way round."""
+    big = inputs.Config("smem_big", 256, (256, 512, 256), B.MLP_ACT_RELU, "exact", 21)
+    small = inputs.Config("smem_small", 16, (256, 512, 256), B.MLP_ACT_RELU, "exact", 22)
+    data = {c.name: oracle_outs(c) for c in (big, small)}
+    pa = B.MlpPipe(big.M, big.widths, big.act, B.make_mode(P))
+    pb = B.MlpPipe(small.M, small.widths, small.act, B.make_mode(P))     # created second: the smaller requirement
+    pc = B.MlpPipe(small.M, small.widths, small.act, B.make_mode(S))
+    try:
+        for p, c in ((pa, big), (pb, small), (pc, small), (pa, big), (pb, small)):
+            X, Ws, outs, _ = data[c.name]
+            Y = p.run(X.cuda(), [w.cuda() for w in Ws])
+            assert np.array_equal(inputs.as_u16(Y.cpu()), outs[-1])
+        assert pa.stats().ready_ok == 1 and pb.stats().ready_ok == 1
+    finally:
+        pa.close(), pb.close(), pc.close()
+
+
 TK = B.MLP_FLAG_TWO_KERNEL
 
 
