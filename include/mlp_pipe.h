@@ -141,10 +141,11 @@ enum {
                                        from mlp_pipe_plan alike).                                                              */
 #define MLP_FLAG_AUTOTUNE 0x400u    /* measured plan search: the FIRST mlp_pipe_run on the handle (outside stream
                                        capture) tries the planner's candidate K-splits / ticket orders (and, unless tile_n is given,
-                                       both unit heights 128 / 256) on the
+                                       both unit heights 128 / 256; for M >= 1024, where they can pay, also CTA pairs as under
+                                       MLP_FLAG_PAIR, if the handle could have been created with that flag) on the
                                        caller's buffers, timing each with the in-kernel clock, and keeps the
                                        fastest.  That one call synchronises the device, may allocate, and takes
-                                       tens of milliseconds; Y is valid after it.  Results are remembered per
+                                       tens of milliseconds (up to a second or two for M in the thousands); Y is valid after it.  Results are remembered per
                                        process for equal (shape, mode).  MICROBATCH candidates are timed from fork to join
                                        with CUDA events (its launches overlap).  If the
                                        first run is being captured into a CUDA graph the search is skipped for good. */

@@ -779,6 +779,23 @@ def test_paper_scale_exact_mode_rasterised_order():
         assert np.array_equal(got, outs[-1]), "Y not bit-exact"
 
 
+def test_autotune_searches_cta_pairs():
+    """MLP_FLAG_AUTOTUNE at M >= 1024 also measures the CTA-pair form of the plan (MLP_FLAG_PAIR) and keeps whichever is
+    faster, so a default handle on the paper's workload gets the fast plan.  Which one wins is a measurement; what must hold
+    either way: the handle that searched AND a second handle that takes the remembered plan agree with the oracle -- bit for
+    bit on an exact-mode shape (where pairs may well lose: the way back from the pair kernel is exercised too), within the
+    tolerance on the paper's shape at M = 1024 (where pairs win by ~7 %)."""
+    tuned = lambda: B.make_mode(P, flags=B.MLP_FLAG_AUTOTUNE)
+    small = inputs.Config("tune_pair_small", 1024, (256, 640, 384), B.MLP_ACT_RELU, "exact", 33)
+    for _ in range(2):
+        st = check(small, tuned())
+        assert st.tile_m == 256 and st.tile_n in (128, 256)
+    st = check(small, B.make_mode(S, flags=B.MLP_FLAG_AUTOTUNE | B.MLP_FLAG_PDL))
+    M = 1024
+    rows = sorted(set(r for b in range(0, M, 256) for r in (b, b + 97 + (b // 256) % 64, b + 255)))
+    _paper_case(M, rows, (tuned(), tuned()))
+
+
 def test_bench_custom_shape_line_is_well_formed():
     """`bench.py --shape ... --pair` (the command behind profiles/paper_workload_r2.md) on a small chain: one JSON line with the
     contract's keys, a tensor- or HBM-bound roofline object and the in-build launch count."""
