@@ -55,6 +55,9 @@ def parse_args():
                     help="M,K,N1,...: a custom chain instead of a BASELINE.json config (e.g. the paper's own workload 16384,8192,8192,8192)")
     ap.add_argument("--act", type=int, default=-1, help="activation for --shape: 0 none, 1 ReLU, 2 GeLU-tanh")
     ap.add_argument("--pair", action="store_true", help="CTA pairs / 2-CTA MMA (MLP_FLAG_PAIR)")
+    ap.add_argument("--no-cooperative", action="store_true",
+                    help="MLP_FLAG_NO_COOPERATIVE: plain instead of cooperative launches (this process has the GPU to itself); what "
+                         "ncu needs to capture the CTA-pair kernel, whose cooperative cluster launch fails under the profiler")
     ap.add_argument("--cublas-ref", action="store_true", help="also time the torch.matmul chain (cuBLAS) on the same inputs: context only")
     ap.add_argument("--no-autotune", action="store_true",
                     help="use the modelled plan instead of the measured plan search of the first (warm-up) run")
@@ -132,7 +135,8 @@ def make_mode(B, args, n_layers):
     split = [int(x) for x in args.split_k.split(",")] if args.split_k else []
     return B.make_mode(kind, chunks=args.chunks if kind == B.MLP_MICROBATCH else 0, sm_split=args.sm_split,
                        stages=args.stages, a_stages=args.a_stages, split_k_layer=split,
-                       flags=(0 if args.no_autotune else B.MLP_FLAG_AUTOTUNE) | (B.MLP_FLAG_PAIR if args.pair else 0))
+                       flags=(0 if args.no_autotune else B.MLP_FLAG_AUTOTUNE) | (B.MLP_FLAG_PAIR if args.pair else 0) |
+                             (B.MLP_FLAG_NO_COOPERATIVE if args.no_cooperative else 0))
 
 
 def max_over_ranks(torch, dist, values, device):
